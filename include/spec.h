@@ -1,0 +1,123 @@
+/*
+ * spec.h — C ABI of the B200 (sm_100a) streaming spectrometer: the GPU-thread hot path of
+ * arXiv 1411.0436 ("the spectrometer implemented in the GPU thread"):
+ *
+ *   int8 complex (dual-pol) samples -> T-tap polyphase pre-filter -> N-point FFT
+ *   -> XX*, YY*, Re(XY*), Im(XY*) -> fp32 accumulation over M spectra
+ *   (PAPER.md:81-83 and the step list PAPER.md:87-96; BASELINE.json north_star names the calls).
+ *
+ * Conventions (DESIGN.md section 3 lists every reading of the paper):
+ *   - one "time sample" is npol complex int8 values: bytes [Xre,Xim,Yre,Yim] (npol=2) or
+ *     [re,im] (npol=1), two's complement, time-major.
+ *   - block b = samples [b*nchan,(b+1)*nchan); spectrum m uses blocks m..m+T-1 (PFB) or block m (FFT).
+ *   - FIR   y[m][n] = sum_{t<T} h[t*nchan+n] * x[(m+t)*nchan+n]
+ *   - DFT   X[k] = sum_n y[n] exp(-2 pi i n k / nchan), unnormalised, DC first
+ *   - out   planar [S][nchan] fp32, S=4: XX, YY, Re(X conj Y), Im(X conj Y); S=1 (npol=1): |X|^2
+ *           summed (not averaged) over nacc consecutive spectra counted from stream start
+ *           (PAPER.md:83,94).
+ * Every function returns an int: >= 0 success, < 0 an SPEC_ERR_* code; on error the handle's
+ * state is unchanged.  No exceptions, no abort.  All calls on one handle come from one host
+ * thread.  Device pointers are plain CUDA device pointers; `cuda_stream` is a cudaStream_t
+ * passed as void* (NULL = the legacy default stream).  The library never falls back to the CPU:
+ * without a CUDA device spec_create fails with SPEC_ERR_CUDA.
+ */
+#ifndef SPEC_H
+#define SPEC_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct spec_ctx spec_t; /* opaque; owned by the library */
+
+enum { SPEC_MODE_PFB = 0, SPEC_MODE_FFT = 1 };
+enum { SPEC_WINDOW_RECT = 0, SPEC_WINDOW_HANN = 1 };
+enum {
+    SPEC_OK = 0,
+    SPEC_ERR_ARG = -1,     /* bad argument value */
+    SPEC_ERR_STATE = -2,   /* call not valid in the handle's current state */
+    SPEC_ERR_SIZE = -3,    /* wrong count / nsamples not a multiple of nchan */
+    SPEC_ERR_OVERRUN = -4, /* the call would complete more accumulations than the ring can hold */
+    SPEC_ERR_CUDA = -5,    /* a CUDA call failed; see spec_last_error() */
+    SPEC_ERR_NOMEM = -6
+};
+
+/* PAPER.md:89-90 (steps 1a/1b: load coefficients, create the FFT plan).
+ * nchan: power of two, 16 <= nchan <= 524288 (the paper's largest).
+ * ntaps: >= 1 (the paper uses 8); ignored (treated as 1) in FFT mode.
+ * npol: 1 or 2.  mode: SPEC_MODE_PFB / SPEC_MODE_FFT (direct FFT).
+ * nacc: spectra per accumulation (>= 1).  window: PFB: h = sinc((k-T*N/2)/N) * w[k], k < T*N,
+ * w = periodic Hann or 1; FFT: h = w over N (RECT = no multiply).  Coefficients are computed in
+ * double on the host and rounded to fp32.  Allocates all device memory (coefficients, twiddles,
+ * history, four-step workspace, a ring of 8 completed accumulations).  *out is set on success. */
+int spec_create(spec_t** out, int nchan, int ntaps, int npol, int mode, long nacc, int window);
+
+/* PAPER.md:89 (step 1a).  Replaces the coefficients: h_coeffs is a HOST array of `count` floats,
+ * count == ntaps*nchan (PFB) or nchan (FFT mode); copied before return (synchronises the device).
+ * SPEC_ERR_SIZE on a wrong count. */
+int spec_set_coeffs(spec_t* s, const float* h_coeffs, size_t count);
+
+/* PAPER.md:91-94 (steps 2-5).  Feeds `nsamples` time samples from DEVICE memory d_in
+ * (nsamples * 2 * npol bytes); nsamples must be a multiple of nchan (0 is a no-op).  The last
+ * (ntaps-1)*nchan samples are carried as filter history to the next call, so results depend only
+ * on the concatenated stream, never on how calls split it.  The history starts empty: the first
+ * spectrum needs ntaps blocks.  All work is queued on cuda_stream; d_in is borrowed until that
+ * work completes.  Returns the number of accumulations completed by this call (>= 0), or
+ * SPEC_ERR_SIZE / SPEC_ERR_OVERRUN (nothing queued) / SPEC_ERR_CUDA. */
+int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* cuda_stream);
+
+/* PAPER.md:95 (step 6).  Pops the oldest completed accumulation into dst as planar
+ * [S][nchan] fp32 in natural channel order.  dst_is_device != 0: dst is device memory and the copy
+ * is only queued on cuda_stream; else dst is host memory and the call returns after the data has
+ * arrived.  Use the stream the producing spec_process used (or synchronise first).
+ * Returns 1, or 0 if nothing is pending. */
+int spec_read_accum(spec_t* s, float* dst, int dst_is_device, void* cuda_stream);
+
+/* Frees everything the handle owns (synchronises the device). */
+int spec_destroy(spec_t* s);
+
+/* ---- small extensions (not named by north_star) ---- */
+
+/* Number of completed accumulations waiting in the ring / spectra produced since start or reset. */
+int spec_pending(const spec_t* s);
+long spec_spectra_done(const spec_t* s);
+
+/* History empty, accumulators zero, ring empty, spectrum counter 0 (synchronises the device). */
+int spec_reset(spec_t* s);
+
+/* Ring capacity (completed accumulations held before SPEC_ERR_OVERRUN); default 8.  Only valid
+ * while nothing is pending and no accumulation is in progress (after create or reset). */
+int spec_set_ring(spec_t* s, int nslots);
+
+/* Copy the coefficients in use to a host array of `count` floats (count as in spec_set_coeffs). */
+int spec_get_coeffs(const spec_t* s, float* h_out, size_t count);
+
+/* PAPER.md:91 + BASELINE.json north_star item (d): streams `nsamples` samples from PINNED HOST
+ * memory in chunks of chunk_samples (a multiple of nchan) through two device buffers: the
+ * host-to-device copy of chunk i+1 runs on a side stream while spec_process works on chunk i on
+ * cuda_stream.  Returns the accumulations completed, like spec_process.  Returns after the last
+ * chunk has been queued; h_pinned must stay valid until cuda_stream has drained. */
+int spec_stream_host(spec_t* s, const void* h_pinned, size_t nsamples, size_t chunk_samples,
+                     void* cuda_stream);
+
+/* Roofline denominator (BASELINE.json north_star: "the measured FP32 peak"): runs a dependent-free
+ * FFMA kernel on every SM and returns the achieved fp32 rate in TFLOP/s (2 flops per FMA). */
+int spec_measure_fp32_peak(double* out_tflops, void* cuda_stream);
+
+/* Test hooks for the bit-exact stages (north_star: "unpack and indexing stages must be bit-exact"):
+ * spec_debug_unpack: d_out[i] = float(int8 d_bytes[i]) for i < nbytes, using the hot path's unpack.
+ * spec_debug_fir: runs the hot path's front end (unpack + FIR, or unpack + window) for ONE
+ * spectrum from d_blocks (ntaps consecutive blocks, device) and writes y as [nchan][2*npol] fp32
+ * (re,im per pol) to d_out (device). */
+int spec_debug_unpack(const void* d_bytes, size_t nbytes, float* d_out, void* cuda_stream);
+int spec_debug_fir(spec_t* s, const void* d_blocks, float* d_out, void* cuda_stream);
+
+const char* spec_strerror(int code);
+const char* spec_last_error(void); /* detail of the last SPEC_ERR_CUDA / SPEC_ERR_NOMEM on this thread */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPEC_H */

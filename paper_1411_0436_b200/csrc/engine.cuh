@@ -1,0 +1,290 @@
+// engine.cuh — the in-CTA FFT engine and the front ends / sinks that make the three hot kernels:
+//   single : unpack + PFB FIR + N-point FFT + Stokes + accumulate            (N <= 4096)
+//   pass A : unpack + PFB FIR + N1-point column FFTs + W_N twiddle -> Z (L2)  (four-step, N > 4096)
+//   pass B : Z -> N2-point row FFTs + Stokes + accumulate
+// PAPER.md:87-96 (section 4, steps 2-5) is the chain; the paper ran it as separate kernels around a
+// cuFFT call on a Kepler card — here the stages are fused so a spectrum never
+// reaches HBM (BASELINE.json north_star items a-c).
+//
+// Engine: in-place decimation-in-frequency FFT of length L = RA*RB*RC over an array A[0..L):
+//   stage a: items ja < LA=L/RA : v[r]=A[ja+r*LA]; DFT_RA; v[q]*=W_L^{ja q}; A[ja+q*LA]=v[q]
+//   stage b: items (qa,jb<LB=LA/RB): v[r]=A[qa*LA+jb+r*LB]; DFT_RB; v[q]*=W_LA^{jb q}; in place
+//   stage c: items (qa,qb)        : v[r]=A[qa*LA+qb*LB+r]; DFT_RC
+// Output frequency k = qa + RA*(qb + RB*qc) sits at position p = qa*LA + qb*LB + qc (digit
+// reversal); accumulators are kept in position order and un-permuted once at read-out.
+// Stage a reads straight from the front end (global memory), the last stage feeds the sink from
+// registers; only the exchanges between stages touch shared memory.
+#pragma once
+#include "fft_math.cuh"
+
+namespace spk {
+
+template <int L_, int RA_, int RB_, int RC_>
+struct Plan {
+    static constexpr int L = L_, RA = RA_, RB = RB_, RC = RC_;
+    static constexpr int NST = (RB_ == 1) ? 1 : ((RC_ == 1) ? 2 : 3);
+    static constexpr int LA = L_ / RA_;
+    static constexpr int LB = LA / RB_;
+    static constexpr int NTS = L_ / 16;  // threads per FFT slot; each thread owns 16 points
+    static constexpr int RLAST = (NST == 1) ? RA_ : ((NST == 2) ? RB_ : RC_);
+    static_assert(RA_ * RB_ * RC_ == L_, "radices must multiply to L");
+    static_assert(L_ >= 16 && RA_ <= 16 && RB_ <= 16 && RC_ <= 16, "16 points per thread");
+};
+
+// ---- input view: the virtual concatenation  history ++ new input
+struct InputView {
+    const uint8_t* hist;  // nhist blocks carried from earlier calls
+    const uint8_t* in;    // this call's samples
+    int nhist;
+};
+
+template <int P>
+__device__ __forceinline__ cpx load_raw(const InputView& v, long long blk, int n, int N) {
+    const uint8_t* base = (blk < v.nhist) ? v.hist + (size_t)blk * N * (2 * P)
+                                          : v.in + (size_t)(blk - v.nhist) * N * (2 * P);
+    if (P == 2) {
+        uint32_t w = __ldg((const uint32_t*)base + n);
+        float xr, xi, yr, yi;
+        unpack4(w, xr, xi, yr, yi);  // bytes [Xre, Xim, Yre, Yim]
+        return {pk(xr, yr), pk(xi, yi)};
+    } else {
+        uint32_t w = __ldg((const uint16_t*)base + n);
+        float xr, xi, d0, d1;
+        unpack4(w, xr, xi, d0, d1);  // bytes [re, im]; upper half unused
+        return {pk(xr, 0.f), pk(xi, 0.f)};
+    }
+}
+
+// front end for `single` and `pass A`: element e of spectrum m is branch n = e*stride + off
+template <int MODE_PFB, int P>
+struct FrontRaw {
+    InputView view;
+    const float* h;  // T*N coefficients (PFB) / N window values or nullptr (FFT mode)
+    int N, T, stride;
+    long long m0;    // spectrum index (in the view) of this launch's job 0
+    __device__ __forceinline__ int off(int slot_id) const { return stride == 1 ? 0 : slot_id; }
+    __device__ __forceinline__ cpx load(long long job, int e, int off_) const {
+        const int n = e * stride + off_;
+        const long long m = m0 + job;
+        if (MODE_PFB) {
+            // y[m][n] = sum_t h[tN+n] x[(m+t)N+n]
+            u64 re = 0ull, im = 0ull;
+            for (int t = 0; t < T; t++) {
+                cpx x = load_raw<P>(view, m + t, n, N);
+                const u64 c = bc(__ldg(h + (size_t)t * N + n));
+                re = fma2(x.re, c, re);
+                im = fma2(x.im, c, im);
+            }
+            return {re, im};
+        } else {
+            cpx x = load_raw<P>(view, m, n, N);
+            if (h) {
+                const u64 c = bc(__ldg(h + n));
+                x.re = mul2(x.re, c);
+                x.im = mul2(x.im, c);
+            }
+            return x;
+        }
+    }
+};
+
+// front end for `pass B`: row `slot_id` of the intermediate Z[m][row][n2] (float4 = Xre,Yre,Xim,Yim)
+struct FrontZ {
+    const float4* Z;
+    int N, N2;
+    __device__ __forceinline__ int off(int slot_id) const { return slot_id; }
+    __device__ __forceinline__ cpx load(long long m, int e, int row) const {
+        const float4 z = Z[(size_t)m * N + (size_t)row * N2 + e];
+        return {pk(z.x, z.y), pk(z.z, z.w)};
+    }
+};
+
+// ---- sinks
+// Stokes detection + accumulation: XX=|X|^2, YY=|Y|^2, Re(X conj Y), Im(X conj Y)
+template <int P>
+struct SinkStokes {
+    float* acc;      // [position][S] fp32, S = 4 (P=2) or 1 (P=1); this accumulation window
+    int slot_len;    // positions per slot (L)
+    int rows_mode;   // 1: slot_id selects a row of the accumulator (pass B); 0: all slots share it
+    struct State {
+        u64 pw[16];
+        float cr[16], ci[16];
+    };
+    __device__ __forceinline__ void begin(State& s) const {
+#pragma unroll
+        for (int i = 0; i < 16; i++) { s.pw[i] = 0ull; s.cr[i] = 0.f; s.ci[i] = 0.f; }
+    }
+    __device__ __forceinline__ void put(State& s, int local, long long, int, int, int, cpx v) const {
+        s.pw[local] = fma2(v.re, v.re, s.pw[local]);
+        s.pw[local] = fma2(v.im, v.im, s.pw[local]);
+        if (P == 2) {
+            float xr, yr, xi, yi;
+            upk(v.re, xr, yr);
+            upk(v.im, xi, yi);
+            s.cr[local] = fmaf(xr, yr, fmaf(xi, yi, s.cr[local]));   // Re(X conj Y) = XrYr + XiYi
+            s.ci[local] = fmaf(xi, yr, fmaf(-xr, yi, s.ci[local]));  // Im(X conj Y) = XiYr - XrYi
+        }
+    }
+    __device__ __forceinline__ void flush(const State& s, int local, int slot_id, int p) const {
+        const size_t pos = (rows_mode ? (size_t)slot_id * slot_len : 0) + p;
+        float xx, yy;
+        upk(s.pw[local], xx, yy);
+        if (P == 2) atomicAdd((float4*)acc + pos, make_float4(xx, yy, s.cr[local], s.ci[local]));
+        else atomicAdd(acc + pos, xx);
+    }
+    static constexpr bool kAccumulates = true;
+};
+
+// pass A sink: multiply by the four-step twiddle W_N^{n2 k1} and store Z[m][p1][n2]
+struct SinkZ {
+    float4* Z;
+    const float2* twN;  // W_N^e, e < N
+    int N, N2;
+    struct State {};
+    __device__ __forceinline__ void begin(State&) const {}
+    __device__ __forceinline__ void put(State&, int, long long m, int n2, int p, int k, cpx v) const {
+        const float2 w = __ldg(twN + (size_t)n2 * k);
+        if (k) v = cmul(v, w.x, w.y);
+        float a, b, c, d;
+        upk(v.re, a, b);
+        upk(v.im, c, d);
+        Z[(size_t)m * N + (size_t)p * N2 + n2] = make_float4(a, b, c, d);
+    }
+    __device__ __forceinline__ void flush(const State&, int, int, int) const {}
+    static constexpr bool kAccumulates = false;
+};
+
+// ---- job map: which spectra a slot processes
+struct JobMap {
+    long long njobs;   // spectra in this launch
+    int len;           // spectra per slot (runs mode) or per blockIdx.y chunk
+    int nslots;        // valid slots (columns / rows / runs)
+    int runs_mode;     // 1: slot_id indexes a run of spectra (single); 0: blockIdx.y does
+};
+
+__device__ __forceinline__ float4 cpx_to_f4(cpx v) {
+    float a, b, c, d;
+    upk(v.re, a, b);
+    upk(v.im, c, d);
+    return make_float4(a, b, c, d);
+}
+__device__ __forceinline__ cpx f4_to_cpx(float4 z) { return {pk(z.x, z.y), pk(z.z, z.w)}; }
+
+// The kernel.  G FFT slots per CTA, PL::NTS threads each.
+//   IL = false ("slot-major"): tid -> slot = tid / NTS, t = tid % NTS; A[p] at slot*L + swz(p)
+//   IL = true  ("interleaved", pass A): slot = tid % G, t = tid / G; A[p] at p*G + slot, so that
+//        adjacent lanes are adjacent columns n2 (coalesced input rows and Z rows, no bank conflicts)
+template <class PL, bool IL, int G, class Front, class Sink>
+__global__ void __launch_bounds__(PL::NTS * G)
+k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __restrict__ twL) {
+    constexpr int L = PL::L, RA = PL::RA, RB = PL::RB, RC = PL::RC, NST = PL::NST;
+    constexpr int LA = PL::LA, LB = PL::LB, NTS = PL::NTS;
+    extern __shared__ float4 smem[];
+
+    const int tid = threadIdx.x;
+    const int slot = IL ? (tid % G) : (tid / NTS);
+    const int t = IL ? (tid / G) : (tid % NTS);
+    const int slot_id = blockIdx.x * G + slot;
+    const bool slot_ok = slot_id < jm.nslots;
+    const long long j0 = (long long)(jm.runs_mode ? slot_id : blockIdx.y) * jm.len;
+    const long long j1 = (j0 + jm.len < jm.njobs) ? j0 + jm.len : jm.njobs;
+    const int off = front.off(slot_id);
+
+    // last-stage swizzle of the slot-major layout: RLAST contiguous points per item, so XOR the low
+    // bits with the item index to spread a quarter-warp over all banks
+    auto addr = [&](int p) -> int {
+        if (IL) return p * G + slot;
+        constexpr int RL = PL::RLAST;
+        const int s = (RL >= 8) ? (p ^ ((p / RL) & 7)) : p;
+        return slot * L + s;
+    };
+
+    typename Sink::State st;
+    sink.begin(st);
+
+    for (int it = 0; it < jm.len; it++) {
+        const long long m = j0 + it;
+        const bool active = slot_ok && (m < j1);
+        // ---------------- stage a
+        if (active) {
+#pragma unroll
+            for (int u = 0; u < 16 / RA; u++) {
+                const int ja = t + NTS * u;
+                cpx v[RA];
+#pragma unroll
+                for (int r = 0; r < RA; r++) v[r] = front.load(m, ja + r * LA, off);
+                dft<RA>(v);
+                if (NST == 1) {
+#pragma unroll
+                    for (int q = 0; q < RA; q++) sink.put(st, u * RA + q, m, off, ja * RA + q, q, v[q]);
+                } else {
+                    smem[addr(ja)] = cpx_to_f4(v[0]);
+#pragma unroll
+                    for (int q = 1; q < RA; q++) {
+                        const float2 w = __ldg(twL + ja * q);
+                        smem[addr(ja + q * LA)] = cpx_to_f4(cmul(v[q], w.x, w.y));
+                    }
+                }
+            }
+        }
+        if (NST >= 2) {
+            __syncthreads();
+            // ---------------- stage b
+            if (active) {
+#pragma unroll
+                for (int u = 0; u < 16 / RB; u++) {
+                    const int i = t + NTS * u;
+                    const int qa = i / LB, jb = i % LB;
+                    const int base = qa * LA + jb;
+                    cpx v[RB];
+#pragma unroll
+                    for (int r = 0; r < RB; r++) v[r] = f4_to_cpx(smem[addr(base + r * LB)]);
+                    dft<RB>(v);
+                    if (NST == 2) {  // LB == 1: i == qa, p = qa*RB + q, k = qa + RA*q
+#pragma unroll
+                        for (int q = 0; q < RB; q++)
+                            sink.put(st, u * RB + q, m, off, i * RB + q, i + RA * q, v[q]);
+                    } else {
+                        smem[addr(base)] = cpx_to_f4(v[0]);
+#pragma unroll
+                        for (int q = 1; q < RB; q++) {
+                            const float2 w = __ldg(twL + RA * jb * q);  // W_LA^{jb q} = W_L^{RA jb q}
+                            smem[addr(base + q * LB)] = cpx_to_f4(cmul(v[q], w.x, w.y));
+                        }
+                    }
+                }
+            }
+            __syncthreads();
+        }
+        if (NST == 3) {
+            // ---------------- stage c
+            if (active) {
+#pragma unroll
+                for (int u = 0; u < 16 / RC; u++) {
+                    const int i = t + NTS * u;  // i = qa*RB + qb
+                    cpx v[RC];
+#pragma unroll
+                    for (int r = 0; r < RC; r++) v[r] = f4_to_cpx(smem[addr(i * RC + r)]);
+                    dft<RC>(v);
+                    const int qa = i / RB, qb = i % RB;
+#pragma unroll
+                    for (int q = 0; q < RC; q++)
+                        sink.put(st, u * RC + q, m, off, i * RC + q, qa + RA * (qb + RB * q), v[q]);
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    if (Sink::kAccumulates && slot_ok && j0 < j1) {
+        constexpr int RL = PL::RLAST;
+#pragma unroll
+        for (int u = 0; u < 16 / RL; u++) {
+            const int i = t + NTS * u;
+#pragma unroll
+            for (int q = 0; q < RL; q++) sink.flush(st, u * RL + q, slot_id, i * RL + q);
+        }
+    }
+}
+
+}  // namespace spk

@@ -1,0 +1,625 @@
+// spec.cu — host side of the C-ABI library declared in include/spec.h: plan, state machine
+// (filter history, accumulation windows, output ring) and kernel launches.  No torch, no CPU
+// fallback: every step of the path runs in the kernels of engine.cuh.
+#include "../../include/spec.h"
+
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <vector>
+
+#include "engine.cuh"
+
+using namespace spk;
+
+// ------------------------------------------------------------------ errors
+static thread_local char g_err[512] = "";
+static int fail_cuda(cudaError_t e, const char* what) {
+    snprintf(g_err, sizeof(g_err), "%s: %s", what, cudaGetErrorString(e));
+    return (e == cudaErrorMemoryAllocation) ? SPEC_ERR_NOMEM : SPEC_ERR_CUDA;
+}
+#define CK(call)                                            \
+    do {                                                    \
+        cudaError_t e__ = (call);                           \
+        if (e__ != cudaSuccess) return fail_cuda(e__, #call); \
+    } while (0)
+
+extern "C" const char* spec_last_error(void) { return g_err; }
+extern "C" const char* spec_strerror(int code) {
+    switch (code) {
+        case SPEC_OK: return "ok";
+        case SPEC_ERR_ARG: return "bad argument";
+        case SPEC_ERR_STATE: return "call not valid in this state";
+        case SPEC_ERR_SIZE: return "wrong size (count, or nsamples not a multiple of nchan)";
+        case SPEC_ERR_OVERRUN: return "output ring overrun: read completed accumulations first";
+        case SPEC_ERR_CUDA: return "CUDA error";
+        case SPEC_ERR_NOMEM: return "out of memory";
+        default: return code > 0 ? "ok" : "unknown error";
+    }
+}
+
+// ------------------------------------------------------------------ handle
+struct spec_ctx {
+    int N, T, P, S, mode, window;
+    long M;
+    int N1, N2;            // four-step split, N1 == 1 for the single-kernel path
+    int numSM;
+    bool use_coef;         // FFT mode: multiply by a window?
+    float* d_coef = nullptr;     // T*N (PFB) or N (FFT)
+    float2* d_twN = nullptr;     // W_N^e (four-step outer twiddle), N entries, only if N1 > 1
+    float2* d_tw1 = nullptr;     // W_N1^e (pass A engine), N1 entries
+    float2* d_tw2 = nullptr;     // W_N2^e (single / pass B engine), N2 entries
+    int* d_perm = nullptr;       // position -> natural channel
+    uint8_t* d_hist[2] = {nullptr, nullptr};
+    int cur = 0, nhist = 0;
+    float4* d_Z = nullptr;       // four-step intermediate, zbatch spectra
+    int zbatch = 0;
+    float* d_ring = nullptr;     // nring accumulators of S*N floats, position order, [pos][S]
+    int nring = 0;
+    float* d_stage = nullptr;    // planar read-out staging, S*N
+    long long count = 0;         // spectra since start/reset
+    long long win_read = 0;      // completed windows already read
+    // streaming helper
+    uint8_t* d_sbuf[2] = {nullptr, nullptr};
+    size_t sbuf_bytes = 0;
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_used[2] = {nullptr, nullptr};
+    std::vector<float> h_coef;
+};
+
+static size_t block_bytes(const spec_ctx* s) { return (size_t)s->N * 2 * s->P; }
+static size_t acc_floats(const spec_ctx* s) { return (size_t)s->S * s->N; }
+static long long windows_done(const spec_ctx* s) { return s->count / s->M; }
+
+// radices of the engine for length L
+static void radices(int L, int r[3]) {
+    switch (L) {
+        case 16: r[0] = 16; r[1] = 1; r[2] = 1; break;
+        case 32: r[0] = 2; r[1] = 16; r[2] = 1; break;
+        case 64: r[0] = 4; r[1] = 16; r[2] = 1; break;
+        case 128: r[0] = 8; r[1] = 16; r[2] = 1; break;
+        case 256: r[0] = 16; r[1] = 16; r[2] = 1; break;
+        case 512: r[0] = 2; r[1] = 16; r[2] = 16; break;
+        case 1024: r[0] = 4; r[1] = 16; r[2] = 16; break;
+        case 2048: r[0] = 8; r[1] = 16; r[2] = 16; break;
+        case 4096: r[0] = 16; r[1] = 16; r[2] = 16; break;
+        default: r[0] = r[1] = r[2] = 1; break;
+    }
+}
+// engine position p -> frequency k (digit reversal, engine.cuh header)
+static int pos_to_freq(int L, int p) {
+    if (L == 1) return 0;
+    int r[3];
+    radices(L, r);
+    const int LA = L / r[0], LB = LA / r[1];
+    const int qa = p / LA, qb = (p % LA) / LB, qc = p % LB;
+    return qa + r[0] * (qb + r[1] * qc);
+}
+
+static void make_twiddles(int L, std::vector<float2>& w) {
+    w.resize(L);
+    for (int e = 0; e < L; e++) {
+        const double a = -2.0 * M_PI * (double)e / (double)L;
+        w[e] = make_float2((float)cos(a), (float)sin(a));
+    }
+}
+
+// default coefficients (include/spec.h spec_create; reading R1)
+static void default_coeffs(const spec_ctx* s, std::vector<float>& h) {
+    const int N = s->N;
+    if (s->mode == SPEC_MODE_FFT) {
+        h.resize(N);
+        for (int k = 0; k < N; k++)
+            h[k] = (s->window == SPEC_WINDOW_HANN) ? (float)(0.5 - 0.5 * cos(2.0 * M_PI * k / (double)N)) : 1.0f;
+        return;
+    }
+    const long Lh = (long)s->T * N;
+    h.resize(Lh);
+    for (long k = 0; k < Lh; k++) {
+        const double x = ((double)k - 0.5 * (double)Lh) / (double)N;
+        const double sinc = (x == 0.0) ? 1.0 : sin(M_PI * x) / (M_PI * x);
+        const double w = (s->window == SPEC_WINDOW_HANN) ? 0.5 - 0.5 * cos(2.0 * M_PI * (double)k / (double)Lh) : 1.0;
+        h[k] = (float)(sinc * w);
+    }
+}
+
+// ------------------------------------------------------------------ small kernels
+// read-out: position order [pos][S] -> planar natural order [S][N]  (PAPER.md:95 step 6)
+__global__ void k_unpermute(const float* __restrict__ acc, const int* __restrict__ perm, float* __restrict__ out,
+                            int N, int S) {
+    const int a = blockIdx.x * blockDim.x + threadIdx.x;
+    if (a >= N) return;
+    const int k = perm[a];
+    if (S == 4) {
+        const float4 v = ((const float4*)acc)[a];
+        out[k] = v.x;
+        out[(size_t)N + k] = v.y;
+        out[(size_t)2 * N + k] = v.z;
+        out[(size_t)3 * N + k] = v.w;
+    } else {
+        out[k] = acc[a];
+    }
+}
+
+__global__ void k_debug_unpack(const uint8_t* __restrict__ b, size_t n, float* __restrict__ out) {
+    const size_t i = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+    if (i >= n) return;
+    uint32_t w = 0;
+    for (int j = 0; j < 4 && i + j < n; j++) w |= (uint32_t)b[i + j] << (8 * j);
+    float f[4];
+    unpack4(w, f[0], f[1], f[2], f[3]);
+    for (int j = 0; j < 4 && i + j < n; j++) out[i + j] = f[j];
+}
+
+template <int MODE_PFB, int P>
+__global__ void k_debug_fir(FrontRaw<MODE_PFB, P> front, float* __restrict__ out) {
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n >= front.N) return;
+    const cpx y = front.load(0, n, 0);
+    float xr, yr, xi, yi;
+    upk(y.re, xr, yr);
+    upk(y.im, xi, yi);
+    if (P == 2) ((float4*)out)[n] = make_float4(xr, xi, yr, yi);
+    else ((float2*)out)[n] = make_float2(xr, xi);
+}
+
+// FP32 peak: 16 independent FFMA chains per thread, operands shared so the register file is not
+// the limit (profiles/r01_ubench.md: 125-128 FMA/clk/SM)
+__global__ void __launch_bounds__(1024, 1) k_fp32_peak(float* out, int iters, float c0, float c1) {
+    float a[16];
+#pragma unroll
+    for (int i = 0; i < 16; i++) a[i] = (float)(threadIdx.x + i) * 1e-9f;
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int i = 0; i < 16; i++) a[i] = fmaf(a[i], c0, c1);
+    }
+    float sum = 0.f;
+#pragma unroll
+    for (int i = 0; i < 16; i++) sum += a[i];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = sum;
+}
+
+// ------------------------------------------------------------------ launches
+template <class K>
+static int prep_smem(K kern, size_t bytes) {
+    if (bytes > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    return 0;
+}
+static inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
+
+template <class PL, int MODE_PFB, int P>
+static int launch_single(spec_ctx* s, const InputView& view, long long m0, long long nspec, float* acc,
+                         cudaStream_t st) {
+    constexpr int G = 256 / PL::NTS;
+    const size_t smem = (PL::NST > 1) ? (size_t)G * PL::L * sizeof(float4) : 0;
+    FrontRaw<MODE_PFB, P> front{view, (MODE_PFB || s->use_coef) ? s->d_coef : nullptr, s->N, s->T, 1, m0};
+    SinkStokes<P> sink{acc, PL::L, 0};
+    const long long target = (long long)s->numSM * 4 * G;
+    const int len = cdiv(nspec, target);
+    const int nruns = cdiv(nspec, len);
+    JobMap jm{nspec, len, nruns, 1};
+    auto kern = k_engine<PL, false, G, FrontRaw<MODE_PFB, P>, SinkStokes<P>>;
+    int rc = prep_smem(kern, smem);
+    if (rc) return rc;
+    kern<<<dim3(cdiv(nruns, G)), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw2);
+    CK(cudaGetLastError());
+    return 0;
+}
+
+template <class PL, int MODE_PFB, int P>
+static int launch_passA(spec_ctx* s, const InputView& view, long long m0, int nb, cudaStream_t st) {
+    constexpr int G = 256 / PL::NTS;
+    const size_t smem = (PL::NST > 1) ? (size_t)G * PL::L * sizeof(float4) : 0;
+    FrontRaw<MODE_PFB, P> front{view, (MODE_PFB || s->use_coef) ? s->d_coef : nullptr, s->N, s->T, s->N2, m0};
+    SinkZ sink{s->d_Z, s->d_twN, s->N, s->N2};
+    const int gx = s->N2 / G;
+    int ny = cdiv((long long)4 * s->numSM, gx);
+    if (ny > nb) ny = nb;
+    const int len = cdiv(nb, ny);
+    ny = cdiv(nb, len);
+    JobMap jm{nb, len, s->N2, 0};
+    auto kern = k_engine<PL, true, G, FrontRaw<MODE_PFB, P>, SinkZ>;
+    int rc = prep_smem(kern, smem);
+    if (rc) return rc;
+    kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw1);
+    CK(cudaGetLastError());
+    return 0;
+}
+
+template <class PL, int P>
+static int launch_passB(spec_ctx* s, int nb, float* acc, cudaStream_t st) {
+    constexpr int G = 256 / PL::NTS;
+    const size_t smem = (size_t)G * PL::L * sizeof(float4);
+    FrontZ front{s->d_Z, s->N, s->N2};
+    SinkStokes<P> sink{acc, PL::L, 1};
+    const int gx = cdiv(s->N1, G);
+    int ny = cdiv((long long)4 * s->numSM, gx);
+    if (ny > nb) ny = nb;
+    const int len = cdiv(nb, ny);
+    ny = cdiv(nb, len);
+    JobMap jm{nb, len, s->N1, 0};
+    auto kern = k_engine<PL, false, G, FrontZ, SinkStokes<P>>;
+    int rc = prep_smem(kern, smem);
+    if (rc) return rc;
+    kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw2);
+    CK(cudaGetLastError());
+    return 0;
+}
+
+typedef Plan<16, 16, 1, 1> PL16;
+typedef Plan<32, 2, 16, 1> PL32;
+typedef Plan<64, 4, 16, 1> PL64;
+typedef Plan<128, 8, 16, 1> PL128;
+typedef Plan<256, 16, 16, 1> PL256;
+typedef Plan<512, 2, 16, 16> PL512;
+typedef Plan<1024, 4, 16, 16> PL1024;
+typedef Plan<2048, 8, 16, 16> PL2048;
+typedef Plan<4096, 16, 16, 16> PL4096;
+
+static int run_single(spec_ctx* s, const InputView& v, long long m0, long long nspec, float* acc, cudaStream_t st) {
+    switch (s->N) {
+#define SINGLE_CASE(LEN, PLX)                                                       \
+    case LEN: {                                                                     \
+        const bool pfb = (s->mode == SPEC_MODE_PFB);                                \
+        if (pfb && s->P == 2) return launch_single<PLX, 1, 2>(s, v, m0, nspec, acc, st); \
+        if (pfb && s->P == 1) return launch_single<PLX, 1, 1>(s, v, m0, nspec, acc, st); \
+        if (!pfb && s->P == 2) return launch_single<PLX, 0, 2>(s, v, m0, nspec, acc, st); \
+        return launch_single<PLX, 0, 1>(s, v, m0, nspec, acc, st);                  \
+    }
+        SINGLE_CASE(16, PL16)
+        SINGLE_CASE(32, PL32)
+        SINGLE_CASE(64, PL64)
+        SINGLE_CASE(128, PL128)
+        SINGLE_CASE(256, PL256)
+        SINGLE_CASE(512, PL512)
+        SINGLE_CASE(1024, PL1024)
+        SINGLE_CASE(2048, PL2048)
+        SINGLE_CASE(4096, PL4096)
+#undef SINGLE_CASE
+    }
+    return SPEC_ERR_ARG;
+}
+
+static int run_passA(spec_ctx* s, const InputView& v, long long m0, int nb, cudaStream_t st) {
+    switch (s->N1) {
+#define A_CASE(LEN, PLX)                                                        \
+    case LEN: {                                                                 \
+        const bool pfb = (s->mode == SPEC_MODE_PFB);                            \
+        if (pfb && s->P == 2) return launch_passA<PLX, 1, 2>(s, v, m0, nb, st); \
+        if (pfb && s->P == 1) return launch_passA<PLX, 1, 1>(s, v, m0, nb, st); \
+        if (!pfb && s->P == 2) return launch_passA<PLX, 0, 2>(s, v, m0, nb, st); \
+        return launch_passA<PLX, 0, 1>(s, v, m0, nb, st);                       \
+    }
+        A_CASE(16, PL16)
+        A_CASE(32, PL32)
+        A_CASE(64, PL64)
+        A_CASE(128, PL128)
+#undef A_CASE
+    }
+    return SPEC_ERR_ARG;
+}
+
+static int run_passB(spec_ctx* s, int nb, float* acc, cudaStream_t st) {
+    switch (s->N2) {
+#define B_CASE(LEN, PLX)                                                   \
+    case LEN:                                                              \
+        return (s->P == 2) ? launch_passB<PLX, 2>(s, nb, acc, st) : launch_passB<PLX, 1>(s, nb, acc, st);
+        B_CASE(512, PL512)
+        B_CASE(1024, PL1024)
+        B_CASE(2048, PL2048)
+        B_CASE(4096, PL4096)
+#undef B_CASE
+    }
+    return SPEC_ERR_ARG;
+}
+
+// `nspec` spectra starting at view-spectrum m0, all inside one accumulation window
+static int run_segment(spec_ctx* s, const InputView& v, long long m0, long long nspec, float* acc, cudaStream_t st) {
+    if (s->N1 == 1) return run_single(s, v, m0, nspec, acc, st);
+    for (long long b0 = 0; b0 < nspec; b0 += s->zbatch) {
+        const int nb = (int)((nspec - b0 < s->zbatch) ? nspec - b0 : s->zbatch);
+        int rc = run_passA(s, v, m0 + b0, nb, st);
+        if (rc) return rc;
+        rc = run_passB(s, nb, acc, st);
+        if (rc) return rc;
+    }
+    return 0;
+}
+
+// ------------------------------------------------------------------ API
+static void free_all(spec_ctx* s) {
+    cudaFree(s->d_coef); cudaFree(s->d_twN); cudaFree(s->d_tw1); cudaFree(s->d_tw2); cudaFree(s->d_perm);
+    cudaFree(s->d_hist[0]); cudaFree(s->d_hist[1]); cudaFree(s->d_Z); cudaFree(s->d_ring); cudaFree(s->d_stage);
+    cudaFree(s->d_sbuf[0]); cudaFree(s->d_sbuf[1]);
+    if (s->side) cudaStreamDestroy(s->side);
+    for (int i = 0; i < 2; i++) {
+        if (s->ev_copied[i]) cudaEventDestroy(s->ev_copied[i]);
+        if (s->ev_used[i]) cudaEventDestroy(s->ev_used[i]);
+    }
+}
+
+static int alloc_ring(spec_ctx* s, int nslots) {
+    float* r = nullptr;
+    CK(cudaMalloc(&r, (size_t)(nslots + 1) * acc_floats(s) * sizeof(float)));
+    cudaFree(s->d_ring);
+    s->d_ring = r;
+    s->nring = nslots + 1;
+    return 0;
+}
+
+static int create_impl(spec_ctx* s) {
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&s->numSM, cudaDevAttrMultiProcessorCount, dev));
+    const int N = s->N;
+    // four-step split: one kernel up to 4096 channels, N1 x N2 beyond
+    if (N <= 4096) { s->N1 = 1; s->N2 = N; }
+    else if (N <= 65536) { s->N1 = 16; s->N2 = N / 16; }
+    else { s->N2 = 4096; s->N1 = N / 4096; }
+
+    default_coeffs(s, s->h_coef);
+    CK(cudaMalloc(&s->d_coef, s->h_coef.size() * sizeof(float)));
+    CK(cudaMemcpy(s->d_coef, s->h_coef.data(), s->h_coef.size() * sizeof(float), cudaMemcpyHostToDevice));
+    s->use_coef = (s->mode == SPEC_MODE_PFB) || (s->window != SPEC_WINDOW_RECT);
+
+    std::vector<float2> w;
+    make_twiddles(s->N2, w);
+    CK(cudaMalloc(&s->d_tw2, w.size() * sizeof(float2)));
+    CK(cudaMemcpy(s->d_tw2, w.data(), w.size() * sizeof(float2), cudaMemcpyHostToDevice));
+    if (s->N1 > 1) {
+        make_twiddles(s->N1, w);
+        CK(cudaMalloc(&s->d_tw1, w.size() * sizeof(float2)));
+        CK(cudaMemcpy(s->d_tw1, w.data(), w.size() * sizeof(float2), cudaMemcpyHostToDevice));
+        make_twiddles(N, w);
+        CK(cudaMalloc(&s->d_twN, w.size() * sizeof(float2)));
+        CK(cudaMemcpy(s->d_twN, w.data(), w.size() * sizeof(float2), cudaMemcpyHostToDevice));
+        size_t zb = ((size_t)32 << 20) / ((size_t)N * sizeof(float4));
+        s->zbatch = (int)(zb < 1 ? 1 : zb);
+        CK(cudaMalloc(&s->d_Z, (size_t)s->zbatch * N * sizeof(float4)));
+    }
+    std::vector<int> perm(N);
+    for (int a = 0; a < N; a++) {
+        const int p1 = a / s->N2, p2 = a % s->N2;
+        perm[a] = pos_to_freq(s->N1, p1) + s->N1 * pos_to_freq(s->N2, p2);
+    }
+    CK(cudaMalloc(&s->d_perm, (size_t)N * sizeof(int)));
+    CK(cudaMemcpy(s->d_perm, perm.data(), (size_t)N * sizeof(int), cudaMemcpyHostToDevice));
+
+    if (s->T > 1) {
+        CK(cudaMalloc(&s->d_hist[0], (size_t)(s->T - 1) * block_bytes(s)));
+        CK(cudaMalloc(&s->d_hist[1], (size_t)(s->T - 1) * block_bytes(s)));
+    }
+    int rc = alloc_ring(s, 8);
+    if (rc) return rc;
+    CK(cudaMalloc(&s->d_stage, acc_floats(s) * sizeof(float)));
+    return 0;
+}
+
+extern "C" int spec_create(spec_t** out, int nchan, int ntaps, int npol, int mode, long nacc, int window) {
+    if (!out) return SPEC_ERR_ARG;
+    if (nchan < 16 || nchan > 524288 || (nchan & (nchan - 1))) return SPEC_ERR_ARG;
+    if (npol != 1 && npol != 2) return SPEC_ERR_ARG;
+    if (mode != SPEC_MODE_PFB && mode != SPEC_MODE_FFT) return SPEC_ERR_ARG;
+    if (window != SPEC_WINDOW_RECT && window != SPEC_WINDOW_HANN) return SPEC_ERR_ARG;
+    if (nacc < 1) return SPEC_ERR_ARG;
+    if (mode == SPEC_MODE_FFT) ntaps = 1;
+    if (ntaps < 1 || ntaps > 64) return SPEC_ERR_ARG;
+    spec_ctx* s = new (std::nothrow) spec_ctx();
+    if (!s) return SPEC_ERR_NOMEM;
+    s->N = nchan; s->T = ntaps; s->P = npol; s->S = (npol == 2) ? 4 : 1;
+    s->mode = mode; s->window = window; s->M = nacc;
+    int rc = create_impl(s);
+    if (rc) { free_all(s); delete s; return rc; }
+    *out = s;
+    return SPEC_OK;
+}
+
+extern "C" int spec_destroy(spec_t* s) {
+    if (!s) return SPEC_ERR_ARG;
+    cudaDeviceSynchronize();
+    free_all(s);
+    delete s;
+    return SPEC_OK;
+}
+
+extern "C" int spec_set_coeffs(spec_t* s, const float* h, size_t count) {
+    if (!s || !h) return SPEC_ERR_ARG;
+    if (count != s->h_coef.size()) return SPEC_ERR_SIZE;
+    CK(cudaDeviceSynchronize());
+    CK(cudaMemcpy(s->d_coef, h, count * sizeof(float), cudaMemcpyHostToDevice));
+    s->h_coef.assign(h, h + count);
+    s->use_coef = true;
+    return SPEC_OK;
+}
+
+extern "C" int spec_get_coeffs(const spec_t* s, float* h_out, size_t count) {
+    if (!s || !h_out) return SPEC_ERR_ARG;
+    if (count != s->h_coef.size()) return SPEC_ERR_SIZE;
+    memcpy(h_out, s->h_coef.data(), count * sizeof(float));
+    return SPEC_OK;
+}
+
+extern "C" int spec_pending(const spec_t* s) { return s ? (int)(windows_done(s) - s->win_read) : SPEC_ERR_ARG; }
+extern "C" long spec_spectra_done(const spec_t* s) { return s ? (long)s->count : SPEC_ERR_ARG; }
+
+extern "C" int spec_reset(spec_t* s) {
+    if (!s) return SPEC_ERR_ARG;
+    CK(cudaDeviceSynchronize());
+    s->nhist = 0; s->cur = 0; s->count = 0; s->win_read = 0;
+    return SPEC_OK;
+}
+
+extern "C" int spec_set_ring(spec_t* s, int nslots) {
+    if (!s || nslots < 1 || nslots > 65536) return SPEC_ERR_ARG;
+    if (s->count != 0 || s->nhist != 0) return SPEC_ERR_STATE;
+    CK(cudaDeviceSynchronize());
+    return alloc_ring(s, nslots);
+}
+
+extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* cuda_stream) {
+    if (!s) return SPEC_ERR_ARG;
+    if (nsamples % (size_t)s->N) return SPEC_ERR_SIZE;
+    if (nsamples == 0) return 0;
+    if (!d_in) return SPEC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const int T = s->T;
+    const long long nblk = (long long)(nsamples / (size_t)s->N);
+    const long long total = s->nhist + nblk;
+    const long long nspec = total >= T ? total - (T - 1) : 0;
+    const long long done_after = (s->count + nspec) / s->M;
+    if (done_after - s->win_read > s->nring - 1) return SPEC_ERR_OVERRUN;
+    const int completed = (int)(done_after - windows_done(s));
+
+    InputView view{s->d_hist[s->cur], (const uint8_t*)d_in, s->nhist};
+    long long i = 0, c = s->count;
+    while (i < nspec) {
+        const long long w = c / s->M;
+        long long take = (w + 1) * s->M - c;
+        if (take > nspec - i) take = nspec - i;
+        float* acc = s->d_ring + (size_t)(w % s->nring) * acc_floats(s);
+        if (c % s->M == 0) CK(cudaMemsetAsync(acc, 0, acc_floats(s) * sizeof(float), st));
+        int rc = run_segment(s, view, i, take, acc, st);
+        if (rc) return rc;
+        i += take;
+        c += take;
+    }
+    // carry the last min(T-1,total) blocks of  history ++ input  (reading R4)
+    const long long keep = total < T - 1 ? total : T - 1;
+    if (keep > 0) {
+        const size_t bb = block_bytes(s);
+        uint8_t* dst = s->d_hist[s->cur ^ 1];
+        const long long first = total - keep;
+        long long nold = s->nhist - first;  // blocks still taken from the old history
+        if (nold < 0) nold = 0;
+        if (nold > 0)
+            CK(cudaMemcpyAsync(dst, s->d_hist[s->cur] + (size_t)first * bb, (size_t)nold * bb,
+                               cudaMemcpyDeviceToDevice, st));
+        const long long nnew = keep - nold;
+        if (nnew > 0)
+            CK(cudaMemcpyAsync(dst + (size_t)nold * bb, (const uint8_t*)d_in + (size_t)(nblk - nnew) * bb,
+                               (size_t)nnew * bb, cudaMemcpyDeviceToDevice, st));
+        s->cur ^= 1;
+    }
+    s->nhist = (int)keep;
+    s->count = c;
+    return completed;
+}
+
+extern "C" int spec_read_accum(spec_t* s, float* dst, int dst_is_device, void* cuda_stream) {
+    if (!s || !dst) return SPEC_ERR_ARG;
+    if (windows_done(s) - s->win_read <= 0) return 0;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const float* acc = s->d_ring + (size_t)(s->win_read % s->nring) * acc_floats(s);
+    float* out = dst_is_device ? dst : s->d_stage;
+    k_unpermute<<<cdiv(s->N, 256), 256, 0, st>>>(acc, s->d_perm, out, s->N, s->S);
+    CK(cudaGetLastError());
+    if (!dst_is_device) {
+        CK(cudaMemcpyAsync(dst, s->d_stage, acc_floats(s) * sizeof(float), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    }
+    s->win_read++;
+    return 1;
+}
+
+extern "C" int spec_stream_host(spec_t* s, const void* h_pinned, size_t nsamples, size_t chunk_samples,
+                                void* cuda_stream) {
+    if (!s || (!h_pinned && nsamples)) return SPEC_ERR_ARG;
+    if (chunk_samples == 0 || chunk_samples % (size_t)s->N || nsamples % (size_t)s->N) return SPEC_ERR_SIZE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t bps = (size_t)2 * s->P;
+    const size_t cbytes = chunk_samples * bps;
+    if (!s->side) {
+        CK(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; i++) {
+            CK(cudaEventCreateWithFlags(&s->ev_copied[i], cudaEventDisableTiming));
+            CK(cudaEventCreateWithFlags(&s->ev_used[i], cudaEventDisableTiming));
+        }
+    }
+    if (s->sbuf_bytes < cbytes) {
+        CK(cudaDeviceSynchronize());
+        for (int i = 0; i < 2; i++) {
+            cudaFree(s->d_sbuf[i]);
+            s->d_sbuf[i] = nullptr;
+            CK(cudaMalloc(&s->d_sbuf[i], cbytes));
+        }
+        s->sbuf_bytes = cbytes;
+        for (int i = 0; i < 2; i++) CK(cudaEventRecord(s->ev_used[i], st));
+    }
+    int completed = 0;
+    size_t done = 0;
+    for (int i = 0; done < nsamples; i++) {
+        const int b = i & 1;
+        const size_t n = (nsamples - done < chunk_samples) ? nsamples - done : chunk_samples;
+        // side stream: wait until the compute stream has finished with this buffer, then copy
+        CK(cudaStreamWaitEvent(s->side, s->ev_used[b], 0));
+        CK(cudaMemcpyAsync(s->d_sbuf[b], (const uint8_t*)h_pinned + done * bps, n * bps, cudaMemcpyHostToDevice,
+                           s->side));
+        CK(cudaEventRecord(s->ev_copied[b], s->side));
+        CK(cudaStreamWaitEvent(st, s->ev_copied[b], 0));
+        const int rc = spec_process(s, s->d_sbuf[b], n, st);
+        if (rc < 0) return rc;
+        completed += rc;
+        CK(cudaEventRecord(s->ev_used[b], st));
+        done += n;
+    }
+    return completed;
+}
+
+extern "C" int spec_measure_fp32_peak(double* out_tflops, void* cuda_stream) {
+    if (!out_tflops) return SPEC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, nsm = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    float* buf = nullptr;
+    CK(cudaMalloc(&buf, (size_t)nsm * 1024 * sizeof(float)));
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    const int iters = 16384;
+    double best = 0.0;
+    for (int rep = 0; rep < 4; rep++) {
+        CK(cudaEventRecord(e0, st));
+        k_fp32_peak<<<nsm, 1024, 0, st>>>(buf, iters, 0.999f, 0.001f);
+        CK(cudaEventRecord(e1, st));
+        CK(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, e0, e1));
+        const double tf = 2.0 * 16.0 * iters * 1024.0 * nsm / (ms * 1e-3) / 1e12;
+        if (rep > 0 && tf > best) best = tf;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(buf);
+    *out_tflops = best;
+    return SPEC_OK;
+}
+
+extern "C" int spec_debug_unpack(const void* d_bytes, size_t nbytes, float* d_out, void* cuda_stream) {
+    if (!d_bytes || !d_out) return SPEC_ERR_ARG;
+    if (nbytes == 0) return SPEC_OK;
+    k_debug_unpack<<<cdiv((long long)((nbytes + 3) / 4), 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+        (const uint8_t*)d_bytes, nbytes, d_out);
+    CK(cudaGetLastError());
+    return SPEC_OK;
+}
+
+extern "C" int spec_debug_fir(spec_t* s, const void* d_blocks, float* d_out, void* cuda_stream) {
+    if (!s || !d_blocks || !d_out) return SPEC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    InputView view{nullptr, (const uint8_t*)d_blocks, 0};
+    const float* h = (s->mode == SPEC_MODE_PFB || s->use_coef) ? s->d_coef : nullptr;
+    const int gx = cdiv(s->N, 256);
+    if (s->mode == SPEC_MODE_PFB) {
+        if (s->P == 2) k_debug_fir<1, 2><<<gx, 256, 0, st>>>(FrontRaw<1, 2>{view, h, s->N, s->T, 1, 0}, d_out);
+        else k_debug_fir<1, 1><<<gx, 256, 0, st>>>(FrontRaw<1, 1>{view, h, s->N, s->T, 1, 0}, d_out);
+    } else {
+        if (s->P == 2) k_debug_fir<0, 2><<<gx, 256, 0, st>>>(FrontRaw<0, 2>{view, h, s->N, s->T, 1, 0}, d_out);
+        else k_debug_fir<0, 1><<<gx, 256, 0, st>>>(FrontRaw<0, 1>{view, h, s->N, s->T, 1, 0}, d_out);
+    }
+    CK(cudaGetLastError());
+    return SPEC_OK;
+}

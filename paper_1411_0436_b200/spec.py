@@ -1,0 +1,145 @@
+"""ctypes binding of include/spec.h — argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; this module holds no
+arithmetic and has no CPU fallback: importing it without the built library raises.
+PyTorch (if the caller uses it) only supplies device memory (`tensor.data_ptr()`) and streams
+(`torch.cuda.current_stream().cuda_stream`); this module itself does not import torch.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libspec.so")
+
+MODE_PFB, MODE_FFT = 0, 1
+WINDOW_RECT, WINDOW_HANN = 0, 1
+OK, ERR_ARG, ERR_STATE, ERR_SIZE, ERR_OVERRUN, ERR_CUDA, ERR_NOMEM = 0, -1, -2, -3, -4, -5, -6
+
+# every symbol include/spec.h declares (tests check the library exports all of them)
+SYMBOLS = [
+    "spec_create", "spec_set_coeffs", "spec_process", "spec_read_accum", "spec_destroy",
+    "spec_pending", "spec_spectra_done", "spec_reset", "spec_set_ring", "spec_get_coeffs",
+    "spec_stream_host", "spec_measure_fp32_peak", "spec_debug_unpack", "spec_debug_fir",
+    "spec_strerror", "spec_last_error",
+]
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(
+        f"{LIB_PATH} is missing: build it with `python -m paper_1411_0436_b200.build` "
+        "(there is no CPU fallback)")
+
+_lib = C.CDLL(LIB_PATH)
+_vp, _sz, _fp = C.c_void_p, C.c_size_t, C.POINTER(C.c_float)
+_lib.spec_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_int, C.c_long, C.c_int]
+_lib.spec_set_coeffs.argtypes = [_vp, _fp, _sz]
+_lib.spec_process.argtypes = [_vp, _vp, _sz, _vp]
+_lib.spec_read_accum.argtypes = [_vp, _vp, C.c_int, _vp]
+_lib.spec_destroy.argtypes = [_vp]
+_lib.spec_pending.argtypes = [_vp]
+_lib.spec_spectra_done.argtypes = [_vp]
+_lib.spec_spectra_done.restype = C.c_long
+_lib.spec_reset.argtypes = [_vp]
+_lib.spec_set_ring.argtypes = [_vp, C.c_int]
+_lib.spec_get_coeffs.argtypes = [_vp, _fp, _sz]
+_lib.spec_stream_host.argtypes = [_vp, _vp, _sz, _sz, _vp]
+_lib.spec_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), _vp]
+_lib.spec_debug_unpack.argtypes = [_vp, _sz, _vp, _vp]
+_lib.spec_debug_fir.argtypes = [_vp, _vp, _vp, _vp]
+_lib.spec_strerror.argtypes = [C.c_int]
+_lib.spec_strerror.restype = C.c_char_p
+_lib.spec_last_error.argtypes = []
+_lib.spec_last_error.restype = C.c_char_p
+
+
+class SpecError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        detail = _lib.spec_last_error().decode() if code in (ERR_CUDA, ERR_NOMEM) else ""
+        super().__init__(f"{where}: {_lib.spec_strerror(code).decode()} ({code}) {detail}".strip())
+
+
+def _check(rc, where):
+    if rc < 0:
+        raise SpecError(rc, where)
+    return rc
+
+
+def strerror(code):
+    return _lib.spec_strerror(code).decode()
+
+
+def measure_fp32_peak(stream=0):
+    out = C.c_double(0.0)
+    _check(_lib.spec_measure_fp32_peak(C.byref(out), stream), "spec_measure_fp32_peak")
+    return out.value
+
+
+def debug_unpack(d_bytes_ptr, nbytes, d_out_ptr, stream=0):
+    _check(_lib.spec_debug_unpack(d_bytes_ptr, nbytes, d_out_ptr, stream), "spec_debug_unpack")
+
+
+class Spec:
+    """Thin handle around spec_t*.  Pointers are integers (device or host addresses)."""
+
+    def __init__(self, nchan, ntaps, npol, mode, nacc, window=WINDOW_HANN):
+        h = _vp()
+        _check(_lib.spec_create(C.byref(h), nchan, ntaps, npol, mode, nacc, window), "spec_create")
+        self._h = h
+        self.nchan, self.npol, self.mode, self.nacc = nchan, npol, mode, nacc
+        self.ntaps = 1 if mode == MODE_FFT else ntaps
+        self.nstokes = 4 if npol == 2 else 1
+        self.ncoef = nchan * self.ntaps
+
+    def set_coeffs(self, h):
+        h = np.ascontiguousarray(h, dtype=np.float32).reshape(-1)
+        _check(_lib.spec_set_coeffs(self._h, h.ctypes.data_as(_fp), h.size), "spec_set_coeffs")
+
+    def get_coeffs(self):
+        out = np.empty(self.ncoef, dtype=np.float32)
+        _check(_lib.spec_get_coeffs(self._h, out.ctypes.data_as(_fp), out.size), "spec_get_coeffs")
+        return out
+
+    def process(self, d_in_ptr, nsamples, stream=0):
+        return _check(_lib.spec_process(self._h, d_in_ptr, nsamples, stream), "spec_process")
+
+    def read_accum_device(self, d_dst_ptr, stream=0):
+        return _check(_lib.spec_read_accum(self._h, d_dst_ptr, 1, stream), "spec_read_accum")
+
+    def read_accum_host(self, stream=0):
+        out = np.empty((self.nstokes, self.nchan), dtype=np.float32)
+        rc = _check(_lib.spec_read_accum(self._h, out.ctypes.data, 0, stream), "spec_read_accum")
+        return out if rc == 1 else None
+
+    def stream_host(self, h_pinned_ptr, nsamples, chunk_samples, stream=0):
+        return _check(_lib.spec_stream_host(self._h, h_pinned_ptr, nsamples, chunk_samples, stream),
+                      "spec_stream_host")
+
+    def pending(self):
+        return _check(_lib.spec_pending(self._h), "spec_pending")
+
+    def spectra_done(self):
+        return _lib.spec_spectra_done(self._h)
+
+    def reset(self):
+        _check(_lib.spec_reset(self._h), "spec_reset")
+
+    def set_ring(self, nslots):
+        _check(_lib.spec_set_ring(self._h, nslots), "spec_set_ring")
+
+    def debug_fir(self, d_blocks_ptr, d_out_ptr, stream=0):
+        _check(_lib.spec_debug_fir(self._h, d_blocks_ptr, d_out_ptr, stream), "spec_debug_fir")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            _lib.spec_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
