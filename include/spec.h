@@ -106,6 +106,14 @@ int spec_stream_host(spec_t* s, const void* h_pinned, size_t nsamples, size_t ch
  * FFMA kernel on every SM and returns the achieved fp32 rate in TFLOP/s (2 flops per FMA). */
 int spec_measure_fp32_peak(double* out_tflops, void* cuda_stream);
 
+/* Per-kernel timing for the roofline report.  spec_profile(s, 1) zeroes the counters and brackets
+ * every later kernel launch with CUDA events on its stream; spec_profile(s, 0) only counts launches.
+ * spec_profile_read waits for the recorded events and returns, per kernel class (0 fused single-pass
+ * kernel, 1 four-step pass A, 2 four-step pass B, 3 read-out un-permute), the summed device time in
+ * ms (0 when timing is off) and the number of launches since the last spec_profile call. */
+int spec_profile(spec_t* s, int enable);
+int spec_profile_read(spec_t* s, double ms[4], long launches[4]);
+
 /* Test hooks for the bit-exact stages (north_star: "unpack and indexing stages must be bit-exact"):
  * spec_debug_unpack: d_out[i] = float(int8 d_bytes[i]) for i < nbytes, using the hot path's unpack.
  * spec_debug_fir: runs the hot path's front end (unpack + FIR, or unpack + window) for ONE

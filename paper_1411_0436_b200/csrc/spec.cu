@@ -68,6 +68,45 @@ struct spec_ctx {
     cudaStream_t side = nullptr;
     cudaEvent_t ev_copied[2] = {nullptr, nullptr}, ev_used[2] = {nullptr, nullptr};
     std::vector<float> h_coef;
+    // optional per-kernel timing (spec_profile): class 0 single, 1 pass A, 2 pass B, 3 read-out
+    bool prof = false;
+    struct Rec { int cls; cudaEvent_t a, b; };
+    std::vector<Rec> recs;
+    std::vector<cudaEvent_t> pool;
+    double prof_ms[4] = {0, 0, 0, 0};
+    long prof_n[4] = {0, 0, 0, 0};
+};
+
+static void prof_fold(spec_ctx* s) {
+    for (auto& r : s->recs) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(r.b) == cudaSuccess && cudaEventElapsedTime(&ms, r.a, r.b) == cudaSuccess)
+            s->prof_ms[r.cls] += ms;
+        s->pool.push_back(r.a);
+        s->pool.push_back(r.b);
+    }
+    s->recs.clear();
+}
+static cudaEvent_t prof_event(spec_ctx* s) {
+    cudaEvent_t e = nullptr;
+    if (!s->pool.empty()) { e = s->pool.back(); s->pool.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+}
+struct ProfScope {
+    spec_ctx* s; cudaStream_t st; cudaEvent_t a = nullptr, b = nullptr; int cls;
+    ProfScope(spec_ctx* s_, int cls_, cudaStream_t st_) : s(s_), st(st_), cls(cls_) {
+        s->prof_n[cls]++;
+        if (!s->prof) return;
+        if (s->recs.size() >= 2048) prof_fold(s);
+        a = prof_event(s); b = prof_event(s);
+        cudaEventRecord(a, st);
+    }
+    ~ProfScope() {
+        if (!a) return;
+        cudaEventRecord(b, st);
+        s->recs.push_back({cls, a, b});
+    }
 };
 
 static size_t block_bytes(const spec_ctx* s) { return (size_t)s->N * 2 * s->P; }
@@ -204,7 +243,10 @@ static int launch_single(spec_ctx* s, const InputView& view, long long m0, long 
     auto kern = k_engine<PL, false, G, FrontRaw<MODE_PFB, P>, SinkStokes<P>>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
-    kern<<<dim3(cdiv(nruns, G)), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw2);
+    {
+        ProfScope ps(s, 0, st);
+        kern<<<dim3(cdiv(nruns, G)), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw2);
+    }
     CK(cudaGetLastError());
     return 0;
 }
@@ -224,7 +266,10 @@ static int launch_passA(spec_ctx* s, const InputView& view, long long m0, int nb
     auto kern = k_engine<PL, true, G, FrontRaw<MODE_PFB, P>, SinkZ>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
-    kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw1);
+    {
+        ProfScope ps(s, 1, st);
+        kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw1);
+    }
     CK(cudaGetLastError());
     return 0;
 }
@@ -244,7 +289,10 @@ static int launch_passB(spec_ctx* s, int nb, float* acc, cudaStream_t st) {
     auto kern = k_engine<PL, false, G, FrontZ, SinkStokes<P>>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
-    kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw2);
+    {
+        ProfScope ps(s, 2, st);
+        kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw2);
+    }
     CK(cudaGetLastError());
     return 0;
 }
@@ -331,6 +379,8 @@ static int run_segment(spec_ctx* s, const InputView& v, long long m0, long long 
 
 // ------------------------------------------------------------------ API
 static void free_all(spec_ctx* s) {
+    prof_fold(s);
+    for (auto e : s->pool) cudaEventDestroy(e);
     cudaFree(s->d_coef); cudaFree(s->d_twN); cudaFree(s->d_tw1); cudaFree(s->d_tw2); cudaFree(s->d_perm);
     cudaFree(s->d_hist[0]); cudaFree(s->d_hist[1]); cudaFree(s->d_Z); cudaFree(s->d_ring); cudaFree(s->d_stage);
     cudaFree(s->d_sbuf[0]); cudaFree(s->d_sbuf[1]);
@@ -514,7 +564,10 @@ extern "C" int spec_read_accum(spec_t* s, float* dst, int dst_is_device, void* c
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const float* acc = s->d_ring + (size_t)(s->win_read % s->nring) * acc_floats(s);
     float* out = dst_is_device ? dst : s->d_stage;
-    k_unpermute<<<cdiv(s->N, 256), 256, 0, st>>>(acc, s->d_perm, out, s->N, s->S);
+    {
+        ProfScope ps(s, 3, st);
+        k_unpermute<<<cdiv(s->N, 256), 256, 0, st>>>(acc, s->d_perm, out, s->N, s->S);
+    }
     CK(cudaGetLastError());
     if (!dst_is_device) {
         CK(cudaMemcpyAsync(dst, s->d_stage, acc_floats(s) * sizeof(float), cudaMemcpyDeviceToHost, st));
@@ -621,5 +674,20 @@ extern "C" int spec_debug_fir(spec_t* s, const void* d_blocks, float* d_out, voi
         else k_debug_fir<0, 1><<<gx, 256, 0, st>>>(FrontRaw<0, 1>{view, h, s->N, s->T, 1, 0}, d_out);
     }
     CK(cudaGetLastError());
+    return SPEC_OK;
+}
+
+extern "C" int spec_profile(spec_t* s, int enable) {
+    if (!s) return SPEC_ERR_ARG;
+    prof_fold(s);
+    s->prof = enable != 0;
+    for (int i = 0; i < 4; i++) { s->prof_ms[i] = 0; s->prof_n[i] = 0; }
+    return SPEC_OK;
+}
+
+extern "C" int spec_profile_read(spec_t* s, double ms[4], long launches[4]) {
+    if (!s || !ms || !launches) return SPEC_ERR_ARG;
+    prof_fold(s);
+    for (int i = 0; i < 4; i++) { ms[i] = s->prof_ms[i]; launches[i] = s->prof_n[i]; }
     return SPEC_OK;
 }

@@ -24,7 +24,7 @@ SYMBOLS = [
     "spec_create", "spec_set_coeffs", "spec_process", "spec_read_accum", "spec_destroy",
     "spec_pending", "spec_spectra_done", "spec_reset", "spec_set_ring", "spec_get_coeffs",
     "spec_stream_host", "spec_measure_fp32_peak", "spec_debug_unpack", "spec_debug_fir",
-    "spec_strerror", "spec_last_error",
+    "spec_strerror", "spec_last_error", "spec_profile", "spec_profile_read",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -49,6 +49,8 @@ _lib.spec_stream_host.argtypes = [_vp, _vp, _sz, _sz, _vp]
 _lib.spec_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), _vp]
 _lib.spec_debug_unpack.argtypes = [_vp, _sz, _vp, _vp]
 _lib.spec_debug_fir.argtypes = [_vp, _vp, _vp, _vp]
+_lib.spec_profile.argtypes = [_vp, C.c_int]
+_lib.spec_profile_read.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_long)]
 _lib.spec_strerror.argtypes = [C.c_int]
 _lib.spec_strerror.restype = C.c_char_p
 _lib.spec_last_error.argtypes = []
@@ -129,6 +131,16 @@ class Spec:
 
     def set_ring(self, nslots):
         _check(_lib.spec_set_ring(self._h, nslots), "spec_set_ring")
+
+    def profile(self, enable=True):
+        _check(_lib.spec_profile(self._h, 1 if enable else 0), "spec_profile")
+
+    def profile_read(self):
+        """{class: (ms, launches)} for classes single, passA, passB, readout."""
+        ms = (C.c_double * 4)()
+        n = (C.c_long * 4)()
+        _check(_lib.spec_profile_read(self._h, ms, n), "spec_profile_read")
+        return {k: (ms[i], n[i]) for i, k in enumerate(("single", "passA", "passB", "readout"))}
 
     def debug_fir(self, d_blocks_ptr, d_out_ptr, stream=0):
         _check(_lib.spec_debug_fir(self._h, d_blocks_ptr, d_out_ptr, stream), "spec_debug_fir")
