@@ -13,7 +13,7 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libspec.so")
 SOURCES = [os.path.join(CSRC, "spec.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("engine.cuh", "fft_math.cuh")] + [
+DEPS = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith((".cu", ".cuh", ".h"))] + [
     os.path.join(_ROOT, "include", "spec.h")]
 
 NVCC_FLAGS = [

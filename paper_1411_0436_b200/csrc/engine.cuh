@@ -38,21 +38,24 @@ struct InputView {
     int nhist;
 };
 
+// one time sample (2*P bytes) of block blk, branch n, as raw bits
 template <int P>
-__device__ __forceinline__ cpx load_raw(const InputView& v, long long blk, int n, int N) {
+__device__ __forceinline__ uint32_t fetch_raw(const InputView& v, long long blk, int n, int N) {
     const uint8_t* base = (blk < v.nhist) ? v.hist + (size_t)blk * N * (2 * P)
                                           : v.in + (size_t)(blk - v.nhist) * N * (2 * P);
-    if (P == 2) {
-        uint32_t w = __ldg((const uint32_t*)base + n);
-        float xr, xi, yr, yi;
-        unpack4(w, xr, xi, yr, yi);  // bytes [Xre, Xim, Yre, Yim]
-        return {pk(xr, yr), pk(xi, yi)};
-    } else {
-        uint32_t w = __ldg((const uint16_t*)base + n);
-        float xr, xi, d0, d1;
-        unpack4(w, xr, xi, d0, d1);  // bytes [re, im]; upper half unused
-        return {pk(xr, 0.f), pk(xi, 0.f)};
-    }
+    if (P == 2) return __ldg((const uint32_t*)base + n);
+    return __ldg((const uint16_t*)base + n);
+}
+template <int P>
+__device__ __forceinline__ cpx unpack_cpx(uint32_t w) {
+    float b0, b1, b2, b3;
+    unpack4(w, b0, b1, b2, b3);
+    if (P == 2) return {pk(b0, b2), pk(b1, b3)};  // bytes [Xre, Xim, Yre, Yim]
+    return {pk(b0, 0.f), pk(b1, 0.f)};            // bytes [re, im]
+}
+template <int P>
+__device__ __forceinline__ cpx load_raw(const InputView& v, long long blk, int n, int N) {
+    return unpack_cpx<P>(fetch_raw<P>(v, blk, n, N));
 }
 
 // front end for `single` and `pass A`: element e of spectrum m is branch n = e*stride + off
@@ -174,8 +177,8 @@ __device__ __forceinline__ cpx f4_to_cpx(float4 z) { return {pk(z.x, z.y), pk(z.
 //   IL = false ("slot-major"): tid -> slot = tid / NTS, t = tid % NTS; A[p] at slot*L + swz(p)
 //   IL = true  ("interleaved", pass A): slot = tid % G, t = tid / G; A[p] at p*G + slot, so that
 //        adjacent lanes are adjacent columns n2 (coalesced input rows and Z rows, no bank conflicts)
-template <class PL, bool IL, int G, class Front, class Sink>
-__global__ void __launch_bounds__(PL::NTS * G)
+template <class PL, bool IL, int G, int MINB, class Front, class Sink>
+__global__ void __launch_bounds__(PL::NTS * G, MINB)
 k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __restrict__ twL) {
     constexpr int L = PL::L, RA = PL::RA, RB = PL::RB, RC = PL::RC, NST = PL::NST;
     constexpr int LA = PL::LA, LB = PL::LB, NTS = PL::NTS;
@@ -221,7 +224,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                     smem[addr(ja)] = cpx_to_f4(v[0]);
 #pragma unroll
                     for (int q = 1; q < RA; q++) {
-                        const float2 w = __ldg(twL + ja * q);
+                        const float2 w = __ldg(twL + (q - 1) * LA + ja);  // W_L^{ja q}, table [q][ja]
                         smem[addr(ja + q * LA)] = cpx_to_f4(cmul(v[q], w.x, w.y));
                     }
                 }
@@ -248,7 +251,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                         smem[addr(base)] = cpx_to_f4(v[0]);
 #pragma unroll
                         for (int q = 1; q < RB; q++) {
-                            const float2 w = __ldg(twL + RA * jb * q);  // W_LA^{jb q} = W_L^{RA jb q}
+                            const float2 w = __ldg(twL + (RA - 1) * LA + (q - 1) * LB + jb);  // W_LA^{jb q}, table [q][jb]
                             smem[addr(base + q * LB)] = cpx_to_f4(cmul(v[q], w.x, w.y));
                         }
                     }

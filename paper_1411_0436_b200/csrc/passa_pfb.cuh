@@ -1,0 +1,85 @@
+// passa_pfb.cuh — four-step pass A for PFB mode with N1 = 16 (8192 <= N <= 65536):
+//   unpack + T-tap FIR for R consecutive spectra -> shared memory -> 16-point column FFTs
+//   -> W_N^{n2 k1} twiddle -> Z[m][k1][n2]  (PAPER.md:92-93 steps 3-4, first FFT factor)
+// A CTA owns C adjacent columns n2 (all 16 rows n1, so 16*C filter branches) and walks a run of
+// spectra R at a time.  FIR phase: each thread owns 16/R branches and slides a T-sample register
+// window over R+T-1 input blocks (every block is loaded and unpacked once per phase; the T-1 halo
+// blocks are re-read from L2 at the next phase).  FFT phase: each thread owns one (spectrum, column)
+// pair: 16 LDS.128, radix-16 in registers, twiddle, 16 coalesced float4 stores.
+#pragma once
+#include "engine.cuh"
+
+namespace spk {
+
+template <int P, int T, int C, int R>
+__global__ void __launch_bounds__(C * R, 2)
+k_passA_pfb16(const InputView view, const float* __restrict__ h, float4* __restrict__ Z,
+              const float2* __restrict__ twN, int N, int N2, long long m0, int nb, int phases_per_cta) {
+    static_assert(16 % R == 0 && T <= 8, "branch split / window size");
+    constexpr int NT = C * R;
+    constexpr int BPT = 16 / R;  // branches per thread
+    extern __shared__ float4 ysm[];  // [R][16][C]
+
+    const int tid = threadIdx.x;
+    const int n2_0 = blockIdx.x * C;
+    const int nphases = (nb + R - 1) / R;
+    const int ph0 = blockIdx.y * phases_per_cta;
+    const int ph1 = (ph0 + phases_per_cta < nphases) ? ph0 + phases_per_cta : nphases;
+
+    // FFT-phase role: spectrum fr of the phase, column fc; its twiddles W_N^{n2 k1} stay in registers
+    const int fr = tid / C, fc = tid % C;
+    const int n2 = n2_0 + fc;
+    float2 tw[16];
+#pragma unroll
+    for (int k = 1; k < 16; k++) tw[k] = __ldg(twN + (size_t)n2 * k);
+
+    for (int ph = ph0; ph < ph1; ph++) {
+        const int j0 = ph * R;  // first job (spectrum) of this phase
+        // ---------------- FIR phase
+#pragma unroll
+        for (int i = 0; i < BPT; i++) {
+            const int beta = tid + NT * i;
+            const int n1 = beta / C, c = beta % C;
+            const int n = n1 * N2 + n2_0 + c;
+            float hc[T];
+#pragma unroll
+            for (int t = 0; t < T; t++) hc[t] = __ldg(h + (size_t)t * N + n);
+            // all R+T-1 blocks of this phase are fetched before any arithmetic (one L2 latency, not R);
+            // in the ragged last phase the block index is clamped to the last valid block
+            const int qmax = nb - 1 - j0 + (T - 1);
+            uint32_t raw[R + T - 1];
+#pragma unroll
+            for (int q = 0; q < R + T - 1; q++)
+                raw[q] = fetch_raw<P>(view, m0 + j0 + (q < qmax ? q : qmax), n, N);
+            cpx x[T];
+#pragma unroll
+            for (int t = 0; t < T - 1; t++) x[t] = unpack_cpx<P>(raw[t]);
+#pragma unroll
+            for (int r = 0; r < R; r++) {
+                x[(r + T - 1) % T] = unpack_cpx<P>(raw[r + T - 1]);
+                u64 re = 0ull, im = 0ull;
+#pragma unroll
+                for (int t = 0; t < T; t++) {
+                    re = fma2(x[(r + t) % T].re, bc(hc[t]), re);
+                    im = fma2(x[(r + t) % T].im, bc(hc[t]), im);
+                }
+                ysm[(r * 16 + n1) * C + c] = cpx_to_f4({re, im});
+            }
+        }
+        __syncthreads();
+        // ---------------- column FFT phase
+        if (j0 + fr < nb) {
+            cpx v[16];
+#pragma unroll
+            for (int n1 = 0; n1 < 16; n1++) v[n1] = f4_to_cpx(ysm[(fr * 16 + n1) * C + fc]);
+            dft<16>(v);
+            float4* zp = Z + (size_t)(j0 + fr) * N + n2;
+            zp[0] = cpx_to_f4(v[0]);
+#pragma unroll
+            for (int k = 1; k < 16; k++) zp[(size_t)k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
+        }
+        __syncthreads();
+    }
+}
+
+}  // namespace spk

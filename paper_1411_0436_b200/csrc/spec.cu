@@ -12,6 +12,7 @@
 #include <vector>
 
 #include "engine.cuh"
+#include "passa_pfb.cuh"
 
 using namespace spk;
 
@@ -138,6 +139,27 @@ static int pos_to_freq(int L, int p) {
     return qa + r[0] * (qb + r[1] * qc);
 }
 
+// engine stage twiddles, laid out [q][j] so that adjacent lanes (adjacent j) read adjacent entries:
+//   stage a: (q-1)*LA + ja -> W_L^{ja q};  stage b (3-stage plans): (RA-1)*LA + (q-1)*LB + jb -> W_LA^{jb q}
+static void make_stage_twiddles(int L, std::vector<float2>& w) {
+    int r[3];
+    radices(L, r);
+    const int LA = L / r[0], LB = LA / r[1];
+    w.clear();
+    if (r[1] == 1) { w.push_back(make_float2(1.f, 0.f)); return; }
+    for (int q = 1; q < r[0]; q++)
+        for (int j = 0; j < LA; j++) {
+            const double a = -2.0 * M_PI * (double)((long)j * q % L) / (double)L;
+            w.push_back(make_float2((float)cos(a), (float)sin(a)));
+        }
+    if (r[2] == 1) return;
+    for (int q = 1; q < r[1]; q++)
+        for (int j = 0; j < LB; j++) {
+            const double a = -2.0 * M_PI * (double)((long)j * q % LA) / (double)LA;
+            w.push_back(make_float2((float)cos(a), (float)sin(a)));
+        }
+}
+
 static void make_twiddles(int L, std::vector<float2>& w) {
     w.resize(L);
     for (int e = 0; e < L; e++) {
@@ -232,7 +254,8 @@ static inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b)
 template <class PL, int MODE_PFB, int P>
 static int launch_single(spec_ctx* s, const InputView& view, long long m0, long long nspec, float* acc,
                          cudaStream_t st) {
-    constexpr int G = 256 / PL::NTS;
+    constexpr int G = (PL::NTS >= 128) ? 1 : 128 / PL::NTS;
+    constexpr int MINB = (PL::NTS * G <= 128) ? 3 : 1;
     const size_t smem = (PL::NST > 1) ? (size_t)G * PL::L * sizeof(float4) : 0;
     FrontRaw<MODE_PFB, P> front{view, (MODE_PFB || s->use_coef) ? s->d_coef : nullptr, s->N, s->T, 1, m0};
     SinkStokes<P> sink{acc, PL::L, 0};
@@ -240,7 +263,7 @@ static int launch_single(spec_ctx* s, const InputView& view, long long m0, long 
     const int len = cdiv(nspec, target);
     const int nruns = cdiv(nspec, len);
     JobMap jm{nspec, len, nruns, 1};
-    auto kern = k_engine<PL, false, G, FrontRaw<MODE_PFB, P>, SinkStokes<P>>;
+    auto kern = k_engine<PL, false, G, MINB, FrontRaw<MODE_PFB, P>, SinkStokes<P>>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
     {
@@ -263,7 +286,7 @@ static int launch_passA(spec_ctx* s, const InputView& view, long long m0, int nb
     const int len = cdiv(nb, ny);
     ny = cdiv(nb, len);
     JobMap jm{nb, len, s->N2, 0};
-    auto kern = k_engine<PL, true, G, FrontRaw<MODE_PFB, P>, SinkZ>;
+    auto kern = k_engine<PL, true, G, 1, FrontRaw<MODE_PFB, P>, SinkZ>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
     {
@@ -276,7 +299,8 @@ static int launch_passA(spec_ctx* s, const InputView& view, long long m0, int nb
 
 template <class PL, int P>
 static int launch_passB(spec_ctx* s, int nb, float* acc, cudaStream_t st) {
-    constexpr int G = 256 / PL::NTS;
+    constexpr int G = (PL::NTS >= 128) ? 1 : 128 / PL::NTS;
+    constexpr int MINB = (PL::NTS * G <= 128) ? 3 : 1;
     const size_t smem = (size_t)G * PL::L * sizeof(float4);
     FrontZ front{s->d_Z, s->N, s->N2};
     SinkStokes<P> sink{acc, PL::L, 1};
@@ -286,7 +310,7 @@ static int launch_passB(spec_ctx* s, int nb, float* acc, cudaStream_t st) {
     const int len = cdiv(nb, ny);
     ny = cdiv(nb, len);
     JobMap jm{nb, len, s->N1, 0};
-    auto kern = k_engine<PL, false, G, FrontZ, SinkStokes<P>>;
+    auto kern = k_engine<PL, false, G, MINB, FrontZ, SinkStokes<P>>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
     {
@@ -331,7 +355,30 @@ static int run_single(spec_ctx* s, const InputView& v, long long m0, long long n
     return SPEC_ERR_ARG;
 }
 
+template <int P>
+static int launch_passA_pfb16(spec_ctx* s, const InputView& view, long long m0, int nb, cudaStream_t st) {
+    constexpr int C = 32, R = 8;
+    const size_t smem = (size_t)R * 16 * C * sizeof(float4);
+    auto kern = k_passA_pfb16<P, 8, C, R>;
+    int rc = prep_smem(kern, smem);
+    if (rc) return rc;
+    const int gx = s->N2 / C;
+    const int nphases = cdiv(nb, R);
+    int ny = cdiv((long long)3 * s->numSM, gx);
+    if (ny > nphases) ny = nphases;
+    const int ppc = cdiv(nphases, ny);
+    ny = cdiv(nphases, ppc);
+    {
+        ProfScope ps(s, 1, st);
+        kern<<<dim3(gx, ny), C * R, smem, st>>>(view, s->d_coef, s->d_Z, s->d_twN, s->N, s->N2, m0, nb, ppc);
+    }
+    CK(cudaGetLastError());
+    return 0;
+}
+
 static int run_passA(spec_ctx* s, const InputView& v, long long m0, int nb, cudaStream_t st) {
+    if (s->mode == SPEC_MODE_PFB && s->N1 == 16 && s->T == 8)
+        return (s->P == 2) ? launch_passA_pfb16<2>(s, v, m0, nb, st) : launch_passA_pfb16<1>(s, v, m0, nb, st);
     switch (s->N1) {
 #define A_CASE(LEN, PLX)                                                        \
     case LEN: {                                                                 \
@@ -416,11 +463,11 @@ static int create_impl(spec_ctx* s) {
     s->use_coef = (s->mode == SPEC_MODE_PFB) || (s->window != SPEC_WINDOW_RECT);
 
     std::vector<float2> w;
-    make_twiddles(s->N2, w);
+    make_stage_twiddles(s->N2, w);
     CK(cudaMalloc(&s->d_tw2, w.size() * sizeof(float2)));
     CK(cudaMemcpy(s->d_tw2, w.data(), w.size() * sizeof(float2), cudaMemcpyHostToDevice));
     if (s->N1 > 1) {
-        make_twiddles(s->N1, w);
+        make_stage_twiddles(s->N1, w);
         CK(cudaMalloc(&s->d_tw1, w.size() * sizeof(float2)));
         CK(cudaMemcpy(s->d_tw1, w.data(), w.size() * sizeof(float2), cudaMemcpyHostToDevice));
         make_twiddles(N, w);
