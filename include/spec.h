@@ -60,7 +60,7 @@ int spec_create(spec_t** out, int nchan, int ntaps, int npol, int mode, long nac
 int spec_set_coeffs(spec_t* s, const float* h_coeffs, size_t count);
 
 /* PAPER.md:91-94 (steps 2-5).  Feeds `nsamples` time samples from DEVICE memory d_in
- * (nsamples * 2 * npol bytes); nsamples must be a multiple of nchan (0 is a no-op).  The last
+ * (nsamples * 2 * npol bytes, 16-byte aligned); nsamples must be a multiple of nchan (0 is a no-op).  The last
  * (ntaps-1)*nchan samples are carried as filter history to the next call, so results depend only
  * on the concatenated stream, never on how calls split it.  The history starts empty: the first
  * spectrum needs ntaps blocks.  All work is queued on cuda_stream; d_in is borrowed until that

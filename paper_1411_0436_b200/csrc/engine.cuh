@@ -31,6 +31,14 @@ struct Plan {
     static_assert(L_ >= 16 && RA_ <= 16 && RB_ <= 16 && RC_ <= 16, "16 points per thread");
 };
 
+__device__ __forceinline__ float4 cpx_to_f4(cpx v) {
+    float a, b, c, d;
+    upk(v.re, a, b);
+    upk(v.im, c, d);
+    return make_float4(a, b, c, d);
+}
+__device__ __forceinline__ cpx f4_to_cpx(float4 z) { return {pk(z.x, z.y), pk(z.z, z.w)}; }
+
 // ---- input view: the virtual concatenation  history ++ new input
 struct InputView {
     const uint8_t* hist;  // nhist blocks carried from earlier calls
@@ -48,9 +56,17 @@ __device__ __forceinline__ uint32_t fetch_raw(const InputView& v, long long blk,
 }
 template <int P>
 __device__ __forceinline__ cpx unpack_cpx(uint32_t w) {
+    if (P == 2) {  // bytes [Xre, Xim, Yre, Yim]: the two magic-number subtractions run as FADD2 on (X,Y) pairs
+        const uint32_t u = w ^ 0x80808080u;
+        const float f0 = __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7440));
+        const float f1 = __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7441));
+        const float f2 = __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7442));
+        const float f3 = __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7443));
+        const u64 k = bc(8388736.0f);
+        return {sub2(pk(f0, f2), k), sub2(pk(f1, f3), k)};
+    }
     float b0, b1, b2, b3;
     unpack4(w, b0, b1, b2, b3);
-    if (P == 2) return {pk(b0, b2), pk(b1, b3)};  // bytes [Xre, Xim, Yre, Yim]
     return {pk(b0, 0.f), pk(b1, 0.f)};            // bytes [re, im]
 }
 template <int P>
@@ -65,6 +81,24 @@ struct FrontRaw {
     const float* h;  // T*N coefficients (PFB) / N window values or nullptr (FFT mode)
     int N, T, stride;
     long long m0;    // spectrum index (in the view) of this launch's job 0
+    // bulk staging (direct-FFT mode, stride 1): one spectrum's raw block is N*2P contiguous bytes
+    static constexpr bool kBulk = (MODE_PFB == 0);
+    static constexpr int kElemBytes = 2 * P;
+    __device__ __forceinline__ const void* src(long long job, int) const {
+        const long long blk = m0 + job;
+        return (blk < view.nhist) ? view.hist + (size_t)blk * N * (2 * P)
+                                  : view.in + (size_t)(blk - view.nhist) * N * (2 * P);
+    }
+    __device__ __forceinline__ cpx decode(const void* x, int e) const {
+        const uint32_t w = (P == 2) ? ((const uint32_t*)x)[e] : (uint32_t)((const uint16_t*)x)[e];
+        cpx v = unpack_cpx<P>(w);
+        if (h) {
+            const u64 c = bc(__ldg(h + e));
+            v.re = mul2(v.re, c);
+            v.im = mul2(v.im, c);
+        }
+        return v;
+    }
     __device__ __forceinline__ int off(int slot_id) const { return stride == 1 ? 0 : slot_id; }
     __device__ __forceinline__ cpx load(long long job, int e, int off_) const {
         const int n = e * stride + off_;
@@ -95,6 +129,12 @@ struct FrontRaw {
 struct FrontZ {
     const float4* Z;
     int N, N2;
+    static constexpr bool kBulk = true;   // one row of one spectrum is N2*16 contiguous bytes
+    static constexpr int kElemBytes = 16;
+    __device__ __forceinline__ const void* src(long long m, int row) const {
+        return Z + (size_t)m * N + (size_t)row * N2;
+    }
+    __device__ __forceinline__ cpx decode(const void* x, int e) const { return f4_to_cpx(((const float4*)x)[e]); }
     __device__ __forceinline__ int off(int slot_id) const { return slot_id; }
     __device__ __forceinline__ cpx load(long long m, int e, int row) const {
         const float4 z = Z[(size_t)m * N + (size_t)row * N2 + e];
@@ -106,7 +146,9 @@ struct FrontZ {
 // Stokes detection + accumulation: XX=|X|^2, YY=|Y|^2, Re(X conj Y), Im(X conj Y)
 template <int P>
 struct SinkStokes {
-    float* acc;      // [position][S] fp32, S = 4 (P=2) or 1 (P=1); this accumulation window
+    float* ring;     // nring accumulators, each [position][S] fp32, S = 4 (P=2) or 1 (P=1)
+    size_t stride;   // floats per accumulator (S*N)
+    int nring;       // accumulation window w lives in ring slot w % nring
     int slot_len;    // positions per slot (L)
     int rows_mode;   // 1: slot_id selects a row of the accumulator (pass B); 0: all slots share it
     struct State {
@@ -128,7 +170,8 @@ struct SinkStokes {
             s.ci[local] = fmaf(xi, yr, fmaf(-xr, yi, s.ci[local]));  // Im(X conj Y) = XiYr - XrYi
         }
     }
-    __device__ __forceinline__ void flush(const State& s, int local, int slot_id, int p) const {
+    __device__ __forceinline__ void flush(const State& s, int local, int slot_id, int p, long long w) const {
+        float* acc = ring + (size_t)(w % nring) * stride;
         const size_t pos = (rows_mode ? (size_t)slot_id * slot_len : 0) + p;
         float xx, yy;
         upk(s.pw[local], xx, yy);
@@ -153,7 +196,7 @@ struct SinkZ {
         upk(v.im, c, d);
         Z[(size_t)m * N + (size_t)p * N2 + n2] = make_float4(a, b, c, d);
     }
-    __device__ __forceinline__ void flush(const State&, int, int, int) const {}
+    __device__ __forceinline__ void flush(const State&, int, int, int, long long) const {}
     static constexpr bool kAccumulates = false;
 };
 
@@ -163,15 +206,10 @@ struct JobMap {
     int len;           // spectra per slot (runs mode) or per blockIdx.y chunk
     int nslots;        // valid slots (columns / rows / runs)
     int runs_mode;     // 1: slot_id indexes a run of spectra (single); 0: blockIdx.y does
+    long long c0;      // spectrum count since stream start at job 0 (accumulation windows)
+    long long M;       // spectra per accumulation window
 };
 
-__device__ __forceinline__ float4 cpx_to_f4(cpx v) {
-    float a, b, c, d;
-    upk(v.re, a, b);
-    upk(v.im, c, d);
-    return make_float4(a, b, c, d);
-}
-__device__ __forceinline__ cpx f4_to_cpx(float4 z) { return {pk(z.x, z.y), pk(z.z, z.w)}; }
 
 // The kernel.  G FFT slots per CTA, PL::NTS threads each.
 //   IL = false ("slot-major"): tid -> slot = tid / NTS, t = tid % NTS; A[p] at slot*L + swz(p)
@@ -183,6 +221,11 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
     constexpr int L = PL::L, RA = PL::RA, RB = PL::RB, RC = PL::RC, NST = PL::NST;
     constexpr int LA = PL::LA, LB = PL::LB, NTS = PL::NTS;
     extern __shared__ float4 smem[];
+    // BULK: the next job's input is copied global -> shared by cp.async.bulk while this job computes
+    constexpr bool BULK = Front::kBulk && !IL && NST >= 2;
+    constexpr int XB = L * Front::kElemBytes;                      // staged bytes per slot
+    uint8_t* xbuf = (uint8_t*)(smem + (size_t)G * L);              // [G][XB]
+    uint64_t* bar = (uint64_t*)(xbuf + (size_t)G * XB);
 
     const int tid = threadIdx.x;
     const int slot = IL ? (tid % G) : (tid / NTS);
@@ -204,10 +247,54 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
 
     typename Sink::State st;
     sink.begin(st);
+    // accumulation window of the current job and the job index at which the next window starts:
+    // a run that crosses a window boundary flushes its partial sums there and starts over
+    long long wcur = (jm.c0 + j0) / jm.M;
+    long long nextb = (wcur + 1) * jm.M - jm.c0;
+    auto flush_all = [&](long long w) {
+        constexpr int RL = PL::RLAST;
+#pragma unroll
+        for (int u = 0; u < 16 / RL; u++) {
+            const int i = t + NTS * u;
+#pragma unroll
+            for (int q = 0; q < RL; q++) sink.flush(st, u * RL + q, slot_id, i * RL + q, w);
+        }
+    };
+
+    // thread 0 issues the copies of iteration `it` for every slot of the CTA
+    auto issue = [&](int it) {
+        uint32_t bytes = 0;
+        for (int g = 0; g < G; g++) {
+            const int sid = blockIdx.x * G + g;
+            const long long gj0 = (long long)(jm.runs_mode ? sid : blockIdx.y) * jm.len;
+            const long long gj1 = (gj0 + jm.len < jm.njobs) ? gj0 + jm.len : jm.njobs;
+            if (sid < jm.nslots && gj0 + it < gj1) bytes += XB;
+        }
+        mbar_expect_tx(bar, bytes);
+        for (int g = 0; g < G; g++) {
+            const int sid = blockIdx.x * G + g;
+            const long long gj0 = (long long)(jm.runs_mode ? sid : blockIdx.y) * jm.len;
+            const long long gj1 = (gj0 + jm.len < jm.njobs) ? gj0 + jm.len : jm.njobs;
+            if (sid < jm.nslots && gj0 + it < gj1)
+                bulk_g2s(xbuf + (size_t)g * XB, front.src(gj0 + it, front.off(sid)), XB, bar);
+        }
+    };
+    if (BULK) {
+        if (tid == 0) mbar_init(bar, 1);
+        __syncthreads();
+        if (tid == 0) issue(0);
+    }
 
     for (int it = 0; it < jm.len; it++) {
         const long long m = j0 + it;
         const bool active = slot_ok && (m < j1);
+        if (BULK) mbar_wait(bar, it & 1);
+        if (Sink::kAccumulates && active && m == nextb) {
+            flush_all(wcur);
+            sink.begin(st);
+            wcur++;
+            nextb += jm.M;
+        }
         // ---------------- stage a
         if (active) {
 #pragma unroll
@@ -215,7 +302,8 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                 const int ja = t + NTS * u;
                 cpx v[RA];
 #pragma unroll
-                for (int r = 0; r < RA; r++) v[r] = front.load(m, ja + r * LA, off);
+                for (int r = 0; r < RA; r++)
+                    v[r] = BULK ? front.decode(xbuf + (size_t)slot * XB, ja + r * LA) : front.load(m, ja + r * LA, off);
                 dft<RA>(v);
                 if (NST == 1) {
 #pragma unroll
@@ -232,6 +320,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
         }
         if (NST >= 2) {
             __syncthreads();
+            if (BULK && tid == 0 && it + 1 < jm.len) issue(it + 1);  // the staging buffer is free again
             // ---------------- stage b
             if (active) {
 #pragma unroll
@@ -279,15 +368,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
         }
     }
 
-    if (Sink::kAccumulates && slot_ok && j0 < j1) {
-        constexpr int RL = PL::RLAST;
-#pragma unroll
-        for (int u = 0; u < 16 / RL; u++) {
-            const int i = t + NTS * u;
-#pragma unroll
-            for (int q = 0; q < RL; q++) sink.flush(st, u * RL + q, slot_id, i * RL + q);
-        }
-    }
+    if (Sink::kAccumulates && slot_ok && j0 < j1) flush_all(wcur);
 }
 
 }  // namespace spk

@@ -36,32 +36,47 @@ k_passA_pfb16(const InputView view, const float* __restrict__ h, float4* __restr
     for (int ph = ph0; ph < ph1; ph++) {
         const int j0 = ph * R;  // first job (spectrum) of this phase
         // ---------------- FIR phase
+        // all (R+T-1) blocks of both branches are fetched before any arithmetic (one L2 latency per
+        // phase); in the ragged last phase the block index is clamped to the last valid block
+        const int qmax = nb - 1 - j0 + (T - 1);
+        uint32_t raw[BPT][R + T - 1];
+        float hc[BPT][T];
+        const bool in_input = (m0 + j0 >= view.nhist);  // no block of this phase comes from the history
+#pragma unroll
+        for (int i = 0; i < BPT; i++) {
+            const int beta = tid + NT * i;
+            const int n = (beta / C) * N2 + n2_0 + (beta % C);
+#pragma unroll
+            for (int t = 0; t < T; t++) hc[i][t] = __ldg(h + (size_t)t * N + n);
+            if (in_input) {
+                const uint8_t* base = view.in + ((size_t)(m0 + j0 - view.nhist) * N + n) * (2 * P);
+                const size_t rowb = (size_t)N * (2 * P);
+#pragma unroll
+                for (int q = 0; q < R + T - 1; q++) {
+                    const uint8_t* p = base + (size_t)(q < qmax ? q : qmax) * rowb;
+                    raw[i][q] = (P == 2) ? __ldg((const uint32_t*)p) : (uint32_t)__ldg((const uint16_t*)p);
+                }
+            } else {
+#pragma unroll
+                for (int q = 0; q < R + T - 1; q++)
+                    raw[i][q] = fetch_raw<P>(view, m0 + j0 + (q < qmax ? q : qmax), n, N);
+            }
+        }
 #pragma unroll
         for (int i = 0; i < BPT; i++) {
             const int beta = tid + NT * i;
             const int n1 = beta / C, c = beta % C;
-            const int n = n1 * N2 + n2_0 + c;
-            float hc[T];
-#pragma unroll
-            for (int t = 0; t < T; t++) hc[t] = __ldg(h + (size_t)t * N + n);
-            // all R+T-1 blocks of this phase are fetched before any arithmetic (one L2 latency, not R);
-            // in the ragged last phase the block index is clamped to the last valid block
-            const int qmax = nb - 1 - j0 + (T - 1);
-            uint32_t raw[R + T - 1];
-#pragma unroll
-            for (int q = 0; q < R + T - 1; q++)
-                raw[q] = fetch_raw<P>(view, m0 + j0 + (q < qmax ? q : qmax), n, N);
             cpx x[T];
 #pragma unroll
-            for (int t = 0; t < T - 1; t++) x[t] = unpack_cpx<P>(raw[t]);
+            for (int t = 0; t < T - 1; t++) x[t] = unpack_cpx<P>(raw[i][t]);
 #pragma unroll
             for (int r = 0; r < R; r++) {
-                x[(r + T - 1) % T] = unpack_cpx<P>(raw[r + T - 1]);
+                x[(r + T - 1) % T] = unpack_cpx<P>(raw[i][r + T - 1]);
                 u64 re = 0ull, im = 0ull;
 #pragma unroll
                 for (int t = 0; t < T; t++) {
-                    re = fma2(x[(r + t) % T].re, bc(hc[t]), re);
-                    im = fma2(x[(r + t) % T].im, bc(hc[t]), im);
+                    re = fma2(x[(r + t) % T].re, bc(hc[i][t]), re);
+                    im = fma2(x[(r + t) % T].im, bc(hc[i][t]), im);
                 }
                 ysm[(r * 16 + n1) * C + c] = cpx_to_f4({re, im});
             }

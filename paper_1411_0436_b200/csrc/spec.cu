@@ -252,17 +252,17 @@ static int prep_smem(K kern, size_t bytes) {
 static inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
 
 template <class PL, int MODE_PFB, int P>
-static int launch_single(spec_ctx* s, const InputView& view, long long m0, long long nspec, float* acc,
+static int launch_single(spec_ctx* s, const InputView& view, long long m0, long long nspec, long long c0,
                          cudaStream_t st) {
     constexpr int G = (PL::NTS >= 128) ? 1 : 128 / PL::NTS;
     constexpr int MINB = (PL::NTS * G <= 128) ? 3 : 1;
-    const size_t smem = (PL::NST > 1) ? (size_t)G * PL::L * sizeof(float4) : 0;
+    const size_t smem = (PL::NST > 1) ? (size_t)G * PL::L * (sizeof(float4) + (MODE_PFB ? 0 : 2 * P)) + 16 : 0;
     FrontRaw<MODE_PFB, P> front{view, (MODE_PFB || s->use_coef) ? s->d_coef : nullptr, s->N, s->T, 1, m0};
-    SinkStokes<P> sink{acc, PL::L, 0};
+    SinkStokes<P> sink{s->d_ring, acc_floats(s), s->nring, PL::L, 0};
     const long long target = (long long)s->numSM * 4 * G;
     const int len = cdiv(nspec, target);
     const int nruns = cdiv(nspec, len);
-    JobMap jm{nspec, len, nruns, 1};
+    JobMap jm{nspec, len, nruns, 1, c0, s->M};
     auto kern = k_engine<PL, false, G, MINB, FrontRaw<MODE_PFB, P>, SinkStokes<P>>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
@@ -285,7 +285,7 @@ static int launch_passA(spec_ctx* s, const InputView& view, long long m0, int nb
     if (ny > nb) ny = nb;
     const int len = cdiv(nb, ny);
     ny = cdiv(nb, len);
-    JobMap jm{nb, len, s->N2, 0};
+    JobMap jm{nb, len, s->N2, 0, 0, 1};
     auto kern = k_engine<PL, true, G, 1, FrontRaw<MODE_PFB, P>, SinkZ>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
@@ -298,18 +298,18 @@ static int launch_passA(spec_ctx* s, const InputView& view, long long m0, int nb
 }
 
 template <class PL, int P>
-static int launch_passB(spec_ctx* s, int nb, float* acc, cudaStream_t st) {
+static int launch_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
     constexpr int G = (PL::NTS >= 128) ? 1 : 128 / PL::NTS;
     constexpr int MINB = (PL::NTS * G <= 128) ? 3 : 1;
-    const size_t smem = (size_t)G * PL::L * sizeof(float4);
+    const size_t smem = (size_t)G * PL::L * 2 * sizeof(float4) + 16;
     FrontZ front{s->d_Z, s->N, s->N2};
-    SinkStokes<P> sink{acc, PL::L, 1};
+    SinkStokes<P> sink{s->d_ring, acc_floats(s), s->nring, PL::L, 1};
     const int gx = cdiv(s->N1, G);
     int ny = cdiv((long long)4 * s->numSM, gx);
     if (ny > nb) ny = nb;
     const int len = cdiv(nb, ny);
     ny = cdiv(nb, len);
-    JobMap jm{nb, len, s->N1, 0};
+    JobMap jm{nb, len, s->N1, 0, c0, s->M};
     auto kern = k_engine<PL, false, G, MINB, FrontZ, SinkStokes<P>>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
@@ -331,15 +331,15 @@ typedef Plan<1024, 4, 16, 16> PL1024;
 typedef Plan<2048, 8, 16, 16> PL2048;
 typedef Plan<4096, 16, 16, 16> PL4096;
 
-static int run_single(spec_ctx* s, const InputView& v, long long m0, long long nspec, float* acc, cudaStream_t st) {
+static int run_single(spec_ctx* s, const InputView& v, long long m0, long long nspec, long long c0, cudaStream_t st) {
     switch (s->N) {
 #define SINGLE_CASE(LEN, PLX)                                                       \
     case LEN: {                                                                     \
         const bool pfb = (s->mode == SPEC_MODE_PFB);                                \
-        if (pfb && s->P == 2) return launch_single<PLX, 1, 2>(s, v, m0, nspec, acc, st); \
-        if (pfb && s->P == 1) return launch_single<PLX, 1, 1>(s, v, m0, nspec, acc, st); \
-        if (!pfb && s->P == 2) return launch_single<PLX, 0, 2>(s, v, m0, nspec, acc, st); \
-        return launch_single<PLX, 0, 1>(s, v, m0, nspec, acc, st);                  \
+        if (pfb && s->P == 2) return launch_single<PLX, 1, 2>(s, v, m0, nspec, c0, st); \
+        if (pfb && s->P == 1) return launch_single<PLX, 1, 1>(s, v, m0, nspec, c0, st); \
+        if (!pfb && s->P == 2) return launch_single<PLX, 0, 2>(s, v, m0, nspec, c0, st); \
+        return launch_single<PLX, 0, 1>(s, v, m0, nspec, c0, st);                  \
     }
         SINGLE_CASE(16, PL16)
         SINGLE_CASE(32, PL32)
@@ -397,11 +397,11 @@ static int run_passA(spec_ctx* s, const InputView& v, long long m0, int nb, cuda
     return SPEC_ERR_ARG;
 }
 
-static int run_passB(spec_ctx* s, int nb, float* acc, cudaStream_t st) {
+static int run_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
     switch (s->N2) {
 #define B_CASE(LEN, PLX)                                                   \
     case LEN:                                                              \
-        return (s->P == 2) ? launch_passB<PLX, 2>(s, nb, acc, st) : launch_passB<PLX, 1>(s, nb, acc, st);
+        return (s->P == 2) ? launch_passB<PLX, 2>(s, nb, c0, st) : launch_passB<PLX, 1>(s, nb, c0, st);
         B_CASE(512, PL512)
         B_CASE(1024, PL1024)
         B_CASE(2048, PL2048)
@@ -411,14 +411,15 @@ static int run_passB(spec_ctx* s, int nb, float* acc, cudaStream_t st) {
     return SPEC_ERR_ARG;
 }
 
-// `nspec` spectra starting at view-spectrum m0, all inside one accumulation window
-static int run_segment(spec_ctx* s, const InputView& v, long long m0, long long nspec, float* acc, cudaStream_t st) {
-    if (s->N1 == 1) return run_single(s, v, m0, nspec, acc, st);
+// `nspec` spectra starting at view-spectrum m0; c0 = spectra produced before them (window bookkeeping
+// is done inside the kernels, so a launch may span accumulation windows)
+static int run_spectra(spec_ctx* s, const InputView& v, long long m0, long long nspec, long long c0, cudaStream_t st) {
+    if (s->N1 == 1) return run_single(s, v, m0, nspec, c0, st);
     for (long long b0 = 0; b0 < nspec; b0 += s->zbatch) {
         const int nb = (int)((nspec - b0 < s->zbatch) ? nspec - b0 : s->zbatch);
         int rc = run_passA(s, v, m0 + b0, nb, st);
         if (rc) return rc;
-        rc = run_passB(s, nb, acc, st);
+        rc = run_passB(s, nb, c0 + b0, st);
         if (rc) return rc;
     }
     return 0;
@@ -473,7 +474,9 @@ static int create_impl(spec_ctx* s) {
         make_twiddles(N, w);
         CK(cudaMalloc(&s->d_twN, w.size() * sizeof(float2)));
         CK(cudaMemcpy(s->d_twN, w.data(), w.size() * sizeof(float2), cudaMemcpyHostToDevice));
-        size_t zb = ((size_t)32 << 20) / ((size_t)N * sizeof(float4));
+        size_t zmb = 32;  // intermediate sized to stay L2-resident; SPEC_ZBATCH_MB overrides
+        if (const char* e = getenv("SPEC_ZBATCH_MB")) { const long v = atol(e); if (v >= 1 && v <= 4096) zmb = (size_t)v; }
+        size_t zb = (zmb << 20) / ((size_t)N * sizeof(float4));
         s->zbatch = (int)(zb < 1 ? 1 : zb);
         CK(cudaMalloc(&s->d_Z, (size_t)s->zbatch * N * sizeof(float4)));
     }
@@ -560,7 +563,7 @@ extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* 
     if (!s) return SPEC_ERR_ARG;
     if (nsamples % (size_t)s->N) return SPEC_ERR_SIZE;
     if (nsamples == 0) return 0;
-    if (!d_in) return SPEC_ERR_ARG;
+    if (!d_in || ((uintptr_t)d_in & 15)) return SPEC_ERR_ARG;  // bulk copies need 16-byte alignment
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const int T = s->T;
     const long long nblk = (long long)(nsamples / (size_t)s->N);
@@ -571,17 +574,21 @@ extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* 
     const int completed = (int)(done_after - windows_done(s));
 
     InputView view{s->d_hist[s->cur], (const uint8_t*)d_in, s->nhist};
-    long long i = 0, c = s->count;
-    while (i < nspec) {
-        const long long w = c / s->M;
-        long long take = (w + 1) * s->M - c;
-        if (take > nspec - i) take = nspec - i;
-        float* acc = s->d_ring + (size_t)(w % s->nring) * acc_floats(s);
-        if (c % s->M == 0) CK(cudaMemsetAsync(acc, 0, acc_floats(s) * sizeof(float), st));
-        int rc = run_segment(s, view, i, take, acc, st);
+    const long long c = s->count + nspec;
+    if (nspec > 0) {
+        // zero the ring slots of every window that starts inside this call (at most two memsets)
+        const long long wfirst = (s->count + s->M - 1) / s->M;  // first window starting at or after count
+        const long long wlast = (c - 1) / s->M;                  // last window touched
+        if (wlast >= wfirst) {
+            const long long nw = wlast - wfirst + 1;
+            const long long s0 = wfirst % s->nring;
+            const long long n0 = (s0 + nw <= s->nring) ? nw : s->nring - s0;
+            const size_t ab = acc_floats(s) * sizeof(float);
+            CK(cudaMemsetAsync(s->d_ring + (size_t)s0 * acc_floats(s), 0, (size_t)n0 * ab, st));
+            if (nw > n0) CK(cudaMemsetAsync(s->d_ring, 0, (size_t)(nw - n0) * ab, st));
+        }
+        int rc = run_spectra(s, view, 0, nspec, s->count, st);
         if (rc) return rc;
-        i += take;
-        c += take;
     }
     // carry the last min(T-1,total) blocks of  history ++ input  (reading R4)
     const long long keep = total < T - 1 ? total : T - 1;
