@@ -75,10 +75,10 @@ __device__ __forceinline__ cpx load_raw(const InputView& v, long long blk, int n
 }
 
 // front end for `single` and `pass A`: element e of spectrum m is branch n = e*stride + off
-template <int MODE_PFB, int P>
+template <int MODE_PFB, int P, int WIN = 1>
 struct FrontRaw {
     InputView view;
-    const float* h;  // T*N coefficients (PFB) / N window values or nullptr (FFT mode)
+    const float* h;  // T*N coefficients (PFB) / N window values (FFT mode, WIN=1; unused when WIN=0)
     int N, T, stride;
     long long m0;    // spectrum index (in the view) of this launch's job 0
     // bulk staging (direct-FFT mode, stride 1): one spectrum's raw block is N*2P contiguous bytes
@@ -92,7 +92,7 @@ struct FrontRaw {
     __device__ __forceinline__ cpx decode(const void* x, int e) const {
         const uint32_t w = (P == 2) ? ((const uint32_t*)x)[e] : (uint32_t)((const uint16_t*)x)[e];
         cpx v = unpack_cpx<P>(w);
-        if (h) {
+        if (WIN) {
             const u64 c = bc(__ldg(h + e));
             v.re = mul2(v.re, c);
             v.im = mul2(v.im, c);
@@ -115,7 +115,7 @@ struct FrontRaw {
             return {re, im};
         } else {
             cpx x = load_raw<P>(view, m, n, N);
-            if (h) {
+            if (WIN) {
                 const u64 c = bc(__ldg(h + n));
                 x.re = mul2(x.re, c);
                 x.im = mul2(x.im, c);
@@ -143,6 +143,9 @@ struct FrontZ {
 };
 
 // ---- sinks
+// The last engine stage hands each sink the 16 outputs of one radix-16 butterfly at once:
+//   put16(state, m, off, i, k0, ks, v): v[q] is the output at engine position p = 16*i + q,
+//   frequency k = k0 + ks*q of the L-point transform, spectrum (job) m, column/row offset `off`.
 // Stokes detection + accumulation: XX=|X|^2, YY=|Y|^2, Re(X conj Y), Im(X conj Y)
 template <int P>
 struct SinkStokes {
@@ -151,34 +154,159 @@ struct SinkStokes {
     int nring;       // accumulation window w lives in ring slot w % nring
     int slot_len;    // positions per slot (L)
     int rows_mode;   // 1: slot_id selects a row of the accumulator (pass B); 0: all slots share it
+    static constexpr bool kAccumulates = true;
+    static constexpr bool kTmem = false;
     struct State {
         u64 pw[16];
         float cr[16], ci[16];
     };
+    __device__ __forceinline__ void init(State&, uint32_t) const {}
     __device__ __forceinline__ void begin(State& s) const {
 #pragma unroll
         for (int i = 0; i < 16; i++) { s.pw[i] = 0ull; s.cr[i] = 0.f; s.ci[i] = 0.f; }
     }
-    __device__ __forceinline__ void put(State& s, int local, long long, int, int, int, cpx v) const {
-        s.pw[local] = fma2(v.re, v.re, s.pw[local]);
-        s.pw[local] = fma2(v.im, v.im, s.pw[local]);
-        if (P == 2) {
-            float xr, yr, xi, yi;
-            upk(v.re, xr, yr);
-            upk(v.im, xi, yi);
-            s.cr[local] = fmaf(xr, yr, fmaf(xi, yi, s.cr[local]));   // Re(X conj Y) = XrYr + XiYi
-            s.ci[local] = fmaf(xi, yr, fmaf(-xr, yi, s.ci[local]));  // Im(X conj Y) = XiYr - XrYi
+    __device__ __forceinline__ void put16(State& s, long long, int, int, int, int, const cpx* v) const {
+#pragma unroll
+        for (int q = 0; q < 16; q++) {
+            s.pw[q] = fma2(v[q].re, v[q].re, s.pw[q]);
+            s.pw[q] = fma2(v[q].im, v[q].im, s.pw[q]);
+            if (P == 2) {
+                float xr, yr, xi, yi;
+                upk(v[q].re, xr, yr);
+                upk(v[q].im, xi, yi);
+                s.cr[q] = fmaf(xr, yr, fmaf(xi, yi, s.cr[q]));   // Re(X conj Y) = XrYr + XiYi
+                s.ci[q] = fmaf(xi, yr, fmaf(-xr, yi, s.ci[q]));  // Im(X conj Y) = XiYr - XrYi
+            }
         }
     }
-    __device__ __forceinline__ void flush(const State& s, int local, int slot_id, int p, long long w) const {
+    // add the partial sums of the 16 positions 16*i .. 16*i+15 to window w's accumulator
+    __device__ __forceinline__ void flush(State& s, int slot_id, int i, long long w) const {
         float* acc = ring + (size_t)(w % nring) * stride;
-        const size_t pos = (rows_mode ? (size_t)slot_id * slot_len : 0) + p;
-        float xx, yy;
-        upk(s.pw[local], xx, yy);
-        if (P == 2) atomicAdd((float4*)acc + pos, make_float4(xx, yy, s.cr[local], s.ci[local]));
-        else atomicAdd(acc + pos, xx);
+        const size_t pos = (rows_mode ? (size_t)slot_id * slot_len : 0) + (size_t)i * 16;
+#pragma unroll
+        for (int q = 0; q < 16; q++) {
+            float xx, yy;
+            upk(s.pw[q], xx, yy);
+            if (P == 2) atomicAdd((float4*)acc + pos + q, make_float4(xx, yy, s.cr[q], s.ci[q]));
+            else atomicAdd(acc + pos + q, xx);
+        }
     }
+};
+
+// ---- tensor memory as accumulator storage (sm_100a).  The 4 Stokes sums of the 16 channels a
+// thread owns are 64 fp32 words that are touched once per spectrum; kept in registers they cost
+// 64 registers per thread and halve the occupancy of the FFT.  TMEM (256 KB per SM, idle here
+// because no tensor-core instruction runs) holds them instead: each thread owns 64 columns of its
+// own TMEM lane (tcgen05.ld/st .32x32b: thread i of a warp <-> lane 32*(warp%4)+i), read-modify-
+// written 32 words at a time around the Stokes FMAs.
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* r) {
+    uint32_t* u = (uint32_t*)r;
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,"
+        "%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        : "=r"(u[0]), "=r"(u[1]), "=r"(u[2]), "=r"(u[3]), "=r"(u[4]), "=r"(u[5]), "=r"(u[6]), "=r"(u[7]),
+          "=r"(u[8]), "=r"(u[9]), "=r"(u[10]), "=r"(u[11]), "=r"(u[12]), "=r"(u[13]), "=r"(u[14]), "=r"(u[15]),
+          "=r"(u[16]), "=r"(u[17]), "=r"(u[18]), "=r"(u[19]), "=r"(u[20]), "=r"(u[21]), "=r"(u[22]), "=r"(u[23]),
+          "=r"(u[24]), "=r"(u[25]), "=r"(u[26]), "=r"(u[27]), "=r"(u[28]), "=r"(u[29]), "=r"(u[30]), "=r"(u[31])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const float* r) {
+    const uint32_t* u = (const uint32_t*)r;
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], "
+        "{%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
+        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+        ::"r"(taddr), "r"(u[0]), "r"(u[1]), "r"(u[2]), "r"(u[3]), "r"(u[4]), "r"(u[5]), "r"(u[6]), "r"(u[7]),
+          "r"(u[8]), "r"(u[9]), "r"(u[10]), "r"(u[11]), "r"(u[12]), "r"(u[13]), "r"(u[14]), "r"(u[15]),
+          "r"(u[16]), "r"(u[17]), "r"(u[18]), "r"(u[19]), "r"(u[20]), "r"(u[21]), "r"(u[22]), "r"(u[23]),
+          "r"(u[24]), "r"(u[25]), "r"(u[26]), "r"(u[27]), "r"(u[28]), "r"(u[29]), "r"(u[30]), "r"(u[31])
+        : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// one warp allocates NCOLS columns (power of two >= 32) for the CTA and publishes the base address
+template <int NCOLS>
+__device__ __forceinline__ uint32_t tmem_alloc_cta(uint32_t* slot_smem) {
+    if (threadIdx.x < 32) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slot_smem)), "n"(NCOLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    return *(volatile uint32_t*)slot_smem;
+}
+template <int NCOLS>
+__device__ __forceinline__ void tmem_free_cta(uint32_t base) {
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (threadIdx.x < 32)
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "n"(NCOLS) : "memory");
+}
+
+// dual-pol Stokes sink with the accumulators in tensor memory: column 4*q+{0,1,2,3} of the thread's
+// lane = XX, YY, Re, Im of its position 16*i+q
+struct SinkStokesTmem {
+    float* ring;
+    size_t stride;
+    int nring;
+    int slot_len;
+    int rows_mode;
     static constexpr bool kAccumulates = true;
+    static constexpr bool kTmem = true;
+    struct State {
+        uint32_t taddr;
+    };
+    __device__ __forceinline__ void init(State& s, uint32_t tmem_base) const {
+        const int warp = threadIdx.x >> 5;
+        s.taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(warp >> 2) * 64;
+    }
+    __device__ __forceinline__ void begin(State& s) const {
+        float z[32];
+#pragma unroll
+        for (int i = 0; i < 32; i++) z[i] = 0.f;
+        tmem_st32(s.taddr, z);
+        tmem_st32(s.taddr + 32, z);
+        tmem_wait_st();
+    }
+    __device__ __forceinline__ void put16(State& s, long long, int, int, int, int, const cpx* v) const {
+#pragma unroll
+        for (int hh = 0; hh < 2; hh++) {
+            float a[32];
+            tmem_ld32(s.taddr + 32 * hh, a);
+            tmem_wait_ld();
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                const cpx x = v[8 * hh + j];
+                u64 pw = pk(a[4 * j], a[4 * j + 1]);
+                pw = fma2(x.re, x.re, pw);
+                pw = fma2(x.im, x.im, pw);
+                upk(pw, a[4 * j], a[4 * j + 1]);
+                float xr, yr, xi, yi;
+                upk(x.re, xr, yr);
+                upk(x.im, xi, yi);
+                a[4 * j + 2] = fmaf(xr, yr, fmaf(xi, yi, a[4 * j + 2]));
+                a[4 * j + 3] = fmaf(xi, yr, fmaf(-xr, yi, a[4 * j + 3]));
+            }
+            tmem_st32(s.taddr + 32 * hh, a);
+        }
+        tmem_wait_st();
+    }
+    __device__ __forceinline__ void flush(State& s, int slot_id, int i, long long w) const {
+        float4* acc = (float4*)(ring + (size_t)(w % nring) * stride);
+        const size_t pos = (rows_mode ? (size_t)slot_id * slot_len : 0) + (size_t)i * 16;
+#pragma unroll
+        for (int hh = 0; hh < 2; hh++) {
+            float a[32];
+            tmem_ld32(s.taddr + 32 * hh, a);
+            tmem_wait_ld();
+#pragma unroll
+            for (int j = 0; j < 8; j++)
+                atomicAdd(acc + pos + 8 * hh + j, make_float4(a[4 * j], a[4 * j + 1], a[4 * j + 2], a[4 * j + 3]));
+        }
+    }
 };
 
 // pass A sink: multiply by the four-step twiddle W_N^{n2 k1} and store Z[m][p1][n2]
@@ -186,18 +314,27 @@ struct SinkZ {
     float4* Z;
     const float2* twN;  // W_N^e, e < N
     int N, N2;
-    struct State {};
-    __device__ __forceinline__ void begin(State&) const {}
-    __device__ __forceinline__ void put(State&, int, long long m, int n2, int p, int k, cpx v) const {
-        const float2 w = __ldg(twN + (size_t)n2 * k);
-        if (k) v = cmul(v, w.x, w.y);
-        float a, b, c, d;
-        upk(v.re, a, b);
-        upk(v.im, c, d);
-        Z[(size_t)m * N + (size_t)p * N2 + n2] = make_float4(a, b, c, d);
-    }
-    __device__ __forceinline__ void flush(const State&, int, int, int, long long) const {}
     static constexpr bool kAccumulates = false;
+    static constexpr bool kTmem = false;
+    struct State {};
+    __device__ __forceinline__ void init(State&, uint32_t) const {}
+    __device__ __forceinline__ void begin(State&) const {}
+    __device__ __forceinline__ void put16(State&, long long m, int n2, int i, int k0, int ks, const cpx* v) const {
+#pragma unroll
+        for (int q = 0; q < 16; q++) {
+            const int k = k0 + ks * q;
+            cpx x = v[q];
+            if (k) {
+                const float2 w = __ldg(twN + (size_t)n2 * k);
+                x = cmul(x, w.x, w.y);
+            }
+            float a, b, c, d;
+            upk(x.re, a, b);
+            upk(x.im, c, d);
+            Z[(size_t)m * N + (size_t)(16 * i + q) * N2 + n2] = make_float4(a, b, c, d);
+        }
+    }
+    __device__ __forceinline__ void flush(State&, int, int, long long) const {}
 };
 
 // ---- job map: which spectra a slot processes
@@ -225,7 +362,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
     constexpr bool BULK = Front::kBulk && !IL && NST >= 2;
     constexpr int XB = L * Front::kElemBytes;                      // staged bytes per slot
     uint8_t* xbuf = (uint8_t*)(smem + (size_t)G * L);              // [G][XB]
-    uint64_t* bar = (uint64_t*)(xbuf + (size_t)G * XB);
+    uint64_t* bar = (uint64_t*)(xbuf + (BULK ? (size_t)G * XB : 0));  // mbarrier, then the TMEM base slot
 
     const int tid = threadIdx.x;
     const int slot = IL ? (tid % G) : (tid / NTS);
@@ -245,21 +382,21 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
         return slot * L + s;
     };
 
+    // TMEM accumulators (SinkStokesTmem): 64 columns per warp-quarter set; needs warp-uniform control
+    // flow around the tcgen05 instructions, i.e. at least one warp per slot
+    constexpr int TCOLS = (NTS * G > 128) ? 128 : 64;
+    static_assert(!Sink::kTmem || NTS >= 32, "TMEM sink: a slot must be at least one warp");
+    uint32_t tmem_base = 0;
+    if (Sink::kTmem) tmem_base = tmem_alloc_cta<TCOLS>((uint32_t*)(bar + 1));
     typename Sink::State st;
+    sink.init(st, tmem_base);
     sink.begin(st);
     // accumulation window of the current job and the job index at which the next window starts:
     // a run that crosses a window boundary flushes its partial sums there and starts over
     long long wcur = (jm.c0 + j0) / jm.M;
     long long nextb = (wcur + 1) * jm.M - jm.c0;
-    auto flush_all = [&](long long w) {
-        constexpr int RL = PL::RLAST;
-#pragma unroll
-        for (int u = 0; u < 16 / RL; u++) {
-            const int i = t + NTS * u;
-#pragma unroll
-            for (int q = 0; q < RL; q++) sink.flush(st, u * RL + q, slot_id, i * RL + q, w);
-        }
-    };
+    static_assert(PL::RLAST == 16, "the last stage is always radix 16 (one put16 per thread and job)");
+    auto flush_all = [&](long long w) { sink.flush(st, slot_id, t, w); };
 
     // thread 0 issues the copies of iteration `it` for every slot of the CTA
     auto issue = [&](int it) {
@@ -307,7 +444,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                 dft<RA>(v);
                 if (NST == 1) {
 #pragma unroll
-                    for (int q = 0; q < RA; q++) sink.put(st, u * RA + q, m, off, ja * RA + q, q, v[q]);
+                    sink.put16(st, m, off, ja, 0, 1, v);
                 } else {
                     smem[addr(ja)] = cpx_to_f4(v[0]);
 #pragma unroll
@@ -333,9 +470,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                     for (int r = 0; r < RB; r++) v[r] = f4_to_cpx(smem[addr(base + r * LB)]);
                     dft<RB>(v);
                     if (NST == 2) {  // LB == 1: i == qa, p = qa*RB + q, k = qa + RA*q
-#pragma unroll
-                        for (int q = 0; q < RB; q++)
-                            sink.put(st, u * RB + q, m, off, i * RB + q, i + RA * q, v[q]);
+                        sink.put16(st, m, off, i, i, RA, v);
                     } else {
                         smem[addr(base)] = cpx_to_f4(v[0]);
 #pragma unroll
@@ -359,9 +494,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                     for (int r = 0; r < RC; r++) v[r] = f4_to_cpx(smem[addr(i * RC + r)]);
                     dft<RC>(v);
                     const int qa = i / RB, qb = i % RB;
-#pragma unroll
-                    for (int q = 0; q < RC; q++)
-                        sink.put(st, u * RC + q, m, off, i * RC + q, qa + RA * (qb + RB * q), v[q]);
+                    sink.put16(st, m, off, i, qa + RA * qb, RA * RB, v);
                 }
             }
             __syncthreads();
@@ -369,6 +502,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
     }
 
     if (Sink::kAccumulates && slot_ok && j0 < j1) flush_all(wcur);
+    if (Sink::kTmem) tmem_free_cta<TCOLS>(tmem_base);
 }
 
 }  // namespace spk

@@ -9,10 +9,12 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <type_traits>
 #include <vector>
 
 #include "engine.cuh"
 #include "passa_pfb.cuh"
+#include "fused.cuh"
 
 using namespace spk;
 
@@ -56,8 +58,12 @@ struct spec_ctx {
     int* d_perm = nullptr;       // position -> natural channel
     uint8_t* d_hist[2] = {nullptr, nullptr};
     int cur = 0, nhist = 0;
-    float4* d_Z = nullptr;       // four-step intermediate, zbatch spectra
+    float4* d_Z = nullptr;       // four-step intermediate, zbatch spectra (fused path: the Z ring)
     int zbatch = 0;
+    // fused persistent four-step kernel (fused.cuh)
+    bool fused = false;
+    int fgrid = 0, fGS = 0, fRING = 0;
+    unsigned* d_flags = nullptr;
     float* d_ring = nullptr;     // nring accumulators of S*N floats, position order, [pos][S]
     int nring = 0;
     float* d_stage = nullptr;    // planar read-out staging, S*N
@@ -215,8 +221,8 @@ __global__ void k_debug_unpack(const uint8_t* __restrict__ b, size_t n, float* _
     for (int j = 0; j < 4 && i + j < n; j++) out[i + j] = f[j];
 }
 
-template <int MODE_PFB, int P>
-__global__ void k_debug_fir(FrontRaw<MODE_PFB, P> front, float* __restrict__ out) {
+template <int MODE_PFB, int P, int WIN>
+__global__ void k_debug_fir(FrontRaw<MODE_PFB, P, WIN> front, float* __restrict__ out) {
     const int n = blockIdx.x * blockDim.x + threadIdx.x;
     if (n >= front.N) return;
     const cpx y = front.load(0, n, 0);
@@ -251,34 +257,57 @@ static int prep_smem(K kern, size_t bytes) {
 }
 static inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
 
-template <class PL, int MODE_PFB, int P>
-static int launch_single(spec_ctx* s, const InputView& view, long long m0, long long nspec, long long c0,
-                         cudaStream_t st) {
+// Stokes sink of the accumulating kernels: dual-pol transforms of at least 512 points (one warp or
+// more per FFT slot) keep their accumulators in tensor memory, everything else in registers
+template <class PL, int P>
+struct StokesSinkOf {
+    static constexpr bool kTmem = (P == 2 && PL::NTS >= 32);
+    typedef typename std::conditional<kTmem, SinkStokesTmem, SinkStokes<P>>::type type;
+};
+static int blocks_by_smem(size_t smem, int cap) {
+    const int b = (int)((227 * 1024) / (smem + 1024));
+    return b < 1 ? 1 : (b > cap ? cap : b);
+}
+
+template <class PL, int MODE_PFB, int P, int WIN>
+static int launch_single_w(spec_ctx* s, const InputView& view, long long m0, long long nspec, long long c0,
+                           cudaStream_t st) {
+    typedef typename StokesSinkOf<PL, P>::type Sink;
+    constexpr bool TM = Sink::kTmem;
     constexpr int G = (PL::NTS >= 128) ? 1 : 128 / PL::NTS;
-    constexpr int MINB = (PL::NTS * G <= 128) ? 3 : 1;
+    constexpr int NT = PL::NTS * G;
+    // register budget: 128 per thread with TMEM accumulators (512 threads per SM), 168 without
+    constexpr int MINB = TM ? 512 / NT : ((NT <= 128) ? 3 : 1);
     const size_t smem = (PL::NST > 1) ? (size_t)G * PL::L * (sizeof(float4) + (MODE_PFB ? 0 : 2 * P)) + 16 : 0;
-    FrontRaw<MODE_PFB, P> front{view, (MODE_PFB || s->use_coef) ? s->d_coef : nullptr, s->N, s->T, 1, m0};
-    SinkStokes<P> sink{s->d_ring, acc_floats(s), s->nring, PL::L, 0};
-    const long long target = (long long)s->numSM * 4 * G;
+    FrontRaw<MODE_PFB, P, WIN> front{view, s->d_coef, s->N, s->T, 1, m0};
+    Sink sink{s->d_ring, acc_floats(s), s->nring, PL::L, 0};
+    const int resident = blocks_by_smem(smem, MINB);
+    const long long target = (long long)s->numSM * resident * 2 * G;
     const int len = cdiv(nspec, target);
     const int nruns = cdiv(nspec, len);
     JobMap jm{nspec, len, nruns, 1, c0, s->M};
-    auto kern = k_engine<PL, false, G, MINB, FrontRaw<MODE_PFB, P>, SinkStokes<P>>;
+    auto kern = k_engine<PL, false, G, MINB, FrontRaw<MODE_PFB, P, WIN>, Sink>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
     {
         ProfScope ps(s, 0, st);
-        kern<<<dim3(cdiv(nruns, G)), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw2);
+        kern<<<dim3(cdiv(nruns, G)), NT, smem, st>>>(front, sink, jm, s->d_tw2);
     }
     CK(cudaGetLastError());
     return 0;
 }
-
 template <class PL, int MODE_PFB, int P>
-static int launch_passA(spec_ctx* s, const InputView& view, long long m0, int nb, cudaStream_t st) {
+static int launch_single(spec_ctx* s, const InputView& view, long long m0, long long nspec, long long c0,
+                         cudaStream_t st) {
+    if (MODE_PFB || s->use_coef) return launch_single_w<PL, MODE_PFB, P, 1>(s, view, m0, nspec, c0, st);
+    return launch_single_w<PL, MODE_PFB, P, 0>(s, view, m0, nspec, c0, st);
+}
+
+template <class PL, int MODE_PFB, int P, int WIN>
+static int launch_passA_w(spec_ctx* s, const InputView& view, long long m0, int nb, cudaStream_t st) {
     constexpr int G = 256 / PL::NTS;
     const size_t smem = (PL::NST > 1) ? (size_t)G * PL::L * sizeof(float4) : 0;
-    FrontRaw<MODE_PFB, P> front{view, (MODE_PFB || s->use_coef) ? s->d_coef : nullptr, s->N, s->T, s->N2, m0};
+    FrontRaw<MODE_PFB, P, WIN> front{view, s->d_coef, s->N, s->T, s->N2, m0};
     SinkZ sink{s->d_Z, s->d_twN, s->N, s->N2};
     const int gx = s->N2 / G;
     int ny = cdiv((long long)4 * s->numSM, gx);
@@ -286,7 +315,7 @@ static int launch_passA(spec_ctx* s, const InputView& view, long long m0, int nb
     const int len = cdiv(nb, ny);
     ny = cdiv(nb, len);
     JobMap jm{nb, len, s->N2, 0, 0, 1};
-    auto kern = k_engine<PL, true, G, 1, FrontRaw<MODE_PFB, P>, SinkZ>;
+    auto kern = k_engine<PL, true, G, 1, FrontRaw<MODE_PFB, P, WIN>, SinkZ>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
     {
@@ -297,25 +326,33 @@ static int launch_passA(spec_ctx* s, const InputView& view, long long m0, int nb
     return 0;
 }
 
+template <class PL, int MODE_PFB, int P>
+static int launch_passA(spec_ctx* s, const InputView& view, long long m0, int nb, cudaStream_t st) {
+    if (MODE_PFB || s->use_coef) return launch_passA_w<PL, MODE_PFB, P, 1>(s, view, m0, nb, st);
+    return launch_passA_w<PL, MODE_PFB, P, 0>(s, view, m0, nb, st);
+}
+
 template <class PL, int P>
 static int launch_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
+    typedef typename StokesSinkOf<PL, P>::type Sink;
     constexpr int G = (PL::NTS >= 128) ? 1 : 128 / PL::NTS;
-    constexpr int MINB = (PL::NTS * G <= 128) ? 3 : 1;
+    constexpr int NT = PL::NTS * G;
+    constexpr int MINB = Sink::kTmem ? 512 / NT : ((NT <= 128) ? 3 : 1);
     const size_t smem = (size_t)G * PL::L * 2 * sizeof(float4) + 16;
     FrontZ front{s->d_Z, s->N, s->N2};
-    SinkStokes<P> sink{s->d_ring, acc_floats(s), s->nring, PL::L, 1};
+    Sink sink{s->d_ring, acc_floats(s), s->nring, PL::L, 1};
     const int gx = cdiv(s->N1, G);
     int ny = cdiv((long long)4 * s->numSM, gx);
     if (ny > nb) ny = nb;
     const int len = cdiv(nb, ny);
     ny = cdiv(nb, len);
     JobMap jm{nb, len, s->N1, 0, c0, s->M};
-    auto kern = k_engine<PL, false, G, MINB, FrontZ, SinkStokes<P>>;
+    auto kern = k_engine<PL, false, G, MINB, FrontZ, Sink>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
     {
         ProfScope ps(s, 2, st);
-        kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw2);
+        kern<<<dim3(gx, ny), NT, smem, st>>>(front, sink, jm, s->d_tw2);
     }
     CK(cudaGetLastError());
     return 0;
@@ -411,10 +448,59 @@ static int run_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
     return SPEC_ERR_ARG;
 }
 
+// ---- fused persistent four-step kernel (fused.cuh): one cooperative launch per call
+template <class PL, int NT, int MODE_PFB>
+static int fused_do(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
+    auto kern = k_fused<PL, NT, MODE_PFB>;
+    const size_t smem = (size_t)NT * 16 * sizeof(float4);
+    if (query) {
+        int rc = prep_smem(kern, smem);
+        if (rc) return rc;
+        int per_sm = 0;
+        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
+        if (per_sm < 1) return SPEC_ERR_CUDA;
+        if (per_sm > 512 / NT) per_sm = 512 / NT;   // tensor memory: 64 (NT=128) / 128 (NT=256) columns per CTA
+        s->fgrid = per_sm * s->numSM;
+        return 0;
+    }
+    FusedParams p;
+    p.view = view; p.h = s->d_coef; p.Z = s->d_Z; p.twN = s->d_twN; p.twL = s->d_tw2;
+    p.ring = s->d_ring; p.acc_stride = acc_floats(s); p.nring = s->nring;
+    p.N = s->N; p.N2 = s->N2; p.nspec = nspec; p.c0 = c0; p.M = s->M;
+    p.GS = s->fGS; p.RING = s->fRING; p.TPG = s->N2 / 16; p.flags = s->d_flags;
+    CK(cudaMemsetAsync(s->d_flags, 0, (size_t)(1 + 2 * s->fRING) * sizeof(unsigned), st));
+    void* args[] = {&p};
+    {
+        ProfScope ps(s, 0, st);
+        CK(cudaLaunchCooperativeKernel((void*)kern, dim3(s->fgrid), dim3(NT), args, smem, st));
+    }
+    return 0;
+}
+
+static int fused_dispatch(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
+    const bool pfb = (s->mode == SPEC_MODE_PFB);
+    switch (s->N2) {
+#define F_CASE(LEN, PLX, NT)                                                         \
+    case LEN:                                                                        \
+        return pfb ? fused_do<PLX, NT, 1>(s, query, view, nspec, c0, st)             \
+                   : fused_do<PLX, NT, 0>(s, query, view, nspec, c0, st);
+        F_CASE(512, PL512, 128)
+        F_CASE(1024, PL1024, 128)
+        F_CASE(2048, PL2048, 128)
+        F_CASE(4096, PL4096, 256)
+#undef F_CASE
+        case 64: return fused_do<PL64, 128, 1>(s, query, view, nspec, c0, st);
+        case 128: return fused_do<PL128, 128, 1>(s, query, view, nspec, c0, st);
+        case 256: return fused_do<PL256, 128, 1>(s, query, view, nspec, c0, st);
+    }
+    return SPEC_ERR_ARG;
+}
+
 // `nspec` spectra starting at view-spectrum m0; c0 = spectra produced before them (window bookkeeping
 // is done inside the kernels, so a launch may span accumulation windows)
 static int run_spectra(spec_ctx* s, const InputView& v, long long m0, long long nspec, long long c0, cudaStream_t st) {
     if (s->N1 == 1) return run_single(s, v, m0, nspec, c0, st);
+    if (s->fused && (s->mode == SPEC_MODE_PFB || !s->use_coef)) return fused_dispatch(s, false, v, nspec, c0, st);
     for (long long b0 = 0; b0 < nspec; b0 += s->zbatch) {
         const int nb = (int)((nspec - b0 < s->zbatch) ? nspec - b0 : s->zbatch);
         int rc = run_passA(s, v, m0 + b0, nb, st);
@@ -431,7 +517,7 @@ static void free_all(spec_ctx* s) {
     for (auto e : s->pool) cudaEventDestroy(e);
     cudaFree(s->d_coef); cudaFree(s->d_twN); cudaFree(s->d_tw1); cudaFree(s->d_tw2); cudaFree(s->d_perm);
     cudaFree(s->d_hist[0]); cudaFree(s->d_hist[1]); cudaFree(s->d_Z); cudaFree(s->d_ring); cudaFree(s->d_stage);
-    cudaFree(s->d_sbuf[0]); cudaFree(s->d_sbuf[1]);
+    cudaFree(s->d_sbuf[0]); cudaFree(s->d_sbuf[1]); cudaFree(s->d_flags);
     if (s->side) cudaStreamDestroy(s->side);
     for (int i = 0; i < 2; i++) {
         if (s->ev_copied[i]) cudaEventDestroy(s->ev_copied[i]);
@@ -454,7 +540,12 @@ static int create_impl(spec_ctx* s) {
     CK(cudaDeviceGetAttribute(&s->numSM, cudaDevAttrMultiProcessorCount, dev));
     const int N = s->N;
     // four-step split: one kernel up to 4096 channels, N1 x N2 beyond
-    if (N <= 4096) { s->N1 = 1; s->N2 = N; }
+    // fused persistent kernel (fused.cuh): dual-pol, 16 x N2, PFB with the paper's 8 taps from 1024
+    // channels (the FIR needs the column split to reuse each unpacked sample), direct FFT from 8192
+    s->fused = s->P == 2 && N >= 1024 && N <= 65536 && !getenv("SPEC_NO_FUSED") &&
+               ((s->mode == SPEC_MODE_PFB && s->T == 8) || (s->mode == SPEC_MODE_FFT && N >= 8192));
+    if (s->fused) { s->N1 = 16; s->N2 = N / 16; }
+    else if (N <= 4096) { s->N1 = 1; s->N2 = N; }
     else if (N <= 65536) { s->N1 = 16; s->N2 = N / 16; }
     else { s->N2 = 4096; s->N1 = N / 4096; }
 
@@ -478,6 +569,21 @@ static int create_impl(spec_ctx* s) {
         if (const char* e = getenv("SPEC_ZBATCH_MB")) { const long v = atol(e); if (v >= 1 && v <= 4096) zmb = (size_t)v; }
         size_t zb = (zmb << 20) / ((size_t)N * sizeof(float4));
         s->zbatch = (int)(zb < 1 ? 1 : zb);
+        if (s->fused) {
+            // ring = two rounds of B jobs (every CTA holds one job of 16*NT points) plus two groups
+            InputView none{nullptr, nullptr, 0};
+            int rc = fused_dispatch(s, true, none, 0, 0, nullptr);
+            if (rc) return rc;
+            const int NT = (s->N2 == 4096) ? 256 : 128;
+            s->fGS = (s->N2 >= 512) ? 16 : 64;
+            if (const char* e = getenv("SPEC_FUSED_GS")) { const int v = atoi(e); if (v >= 1 && v <= 4096) s->fGS = v; }
+            const long long round_spectra = ((long long)s->fgrid * NT * 16 + N - 1) / N;
+            long long rs = 2 * round_spectra + 2 * s->fGS;
+            s->fRING = (int)((rs + s->fGS - 1) / s->fGS);
+            if (const char* e = getenv("SPEC_FUSED_RING")) { const int v = atoi(e); if (v >= 2 && v <= 4096) s->fRING = v; }
+            s->zbatch = s->fRING * s->fGS;
+            CK(cudaMalloc(&s->d_flags, (size_t)(1 + 2 * s->fRING) * sizeof(unsigned)));
+        }
         CK(cudaMalloc(&s->d_Z, (size_t)s->zbatch * N * sizeof(float4)));
     }
     std::vector<int> perm(N);
@@ -718,14 +824,17 @@ extern "C" int spec_debug_fir(spec_t* s, const void* d_blocks, float* d_out, voi
     if (!s || !d_blocks || !d_out) return SPEC_ERR_ARG;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     InputView view{nullptr, (const uint8_t*)d_blocks, 0};
-    const float* h = (s->mode == SPEC_MODE_PFB || s->use_coef) ? s->d_coef : nullptr;
+    const float* h = s->d_coef;
     const int gx = cdiv(s->N, 256);
     if (s->mode == SPEC_MODE_PFB) {
-        if (s->P == 2) k_debug_fir<1, 2><<<gx, 256, 0, st>>>(FrontRaw<1, 2>{view, h, s->N, s->T, 1, 0}, d_out);
-        else k_debug_fir<1, 1><<<gx, 256, 0, st>>>(FrontRaw<1, 1>{view, h, s->N, s->T, 1, 0}, d_out);
+        if (s->P == 2) k_debug_fir<1, 2, 1><<<gx, 256, 0, st>>>(FrontRaw<1, 2, 1>{view, h, s->N, s->T, 1, 0}, d_out);
+        else k_debug_fir<1, 1, 1><<<gx, 256, 0, st>>>(FrontRaw<1, 1, 1>{view, h, s->N, s->T, 1, 0}, d_out);
+    } else if (s->use_coef) {
+        if (s->P == 2) k_debug_fir<0, 2, 1><<<gx, 256, 0, st>>>(FrontRaw<0, 2, 1>{view, h, s->N, s->T, 1, 0}, d_out);
+        else k_debug_fir<0, 1, 1><<<gx, 256, 0, st>>>(FrontRaw<0, 1, 1>{view, h, s->N, s->T, 1, 0}, d_out);
     } else {
-        if (s->P == 2) k_debug_fir<0, 2><<<gx, 256, 0, st>>>(FrontRaw<0, 2>{view, h, s->N, s->T, 1, 0}, d_out);
-        else k_debug_fir<0, 1><<<gx, 256, 0, st>>>(FrontRaw<0, 1>{view, h, s->N, s->T, 1, 0}, d_out);
+        if (s->P == 2) k_debug_fir<0, 2, 0><<<gx, 256, 0, st>>>(FrontRaw<0, 2, 0>{view, h, s->N, s->T, 1, 0}, d_out);
+        else k_debug_fir<0, 1, 0><<<gx, 256, 0, st>>>(FrontRaw<0, 1, 0>{view, h, s->N, s->T, 1, 0}, d_out);
     }
     CK(cudaGetLastError());
     return SPEC_OK;

@@ -106,6 +106,47 @@ def test_parity_random_bytes_all_kernels(nchan, mode, npol):
         check_stokes_invariants(a)
 
 
+FUSED_SIZES = [1024, 2048, 4096, 8192, 16384, 32768, 65536]
+
+
+@pytest.mark.parametrize("mode", [PFB, FFT])
+@pytest.mark.parametrize("nchan", FUSED_SIZES)
+def test_parity_fused_persistent_kernel_small_streams(nchan, mode):
+    """The persistent four-step kernel (dual-pol, 8 taps / rectangular direct FFT): full-range random
+    bytes, arbitrary PFB coefficients, a ragged last group, windows that straddle three unequal calls."""
+    T = 8 if mode == PFB else 1
+    M = 3
+    nblk = 2 * M + (T - 1) + 2
+    raw = synth.random_bytes(nchan * 5 + mode, nblk * nchan, 2)
+    h = synth.random_coeffs(nchan + 2, nchan * T) if mode == PFB else None
+    splits = [nchan * 2, nchan * (nblk - 5), nchan * 3]
+    g, gd = gpu_run(raw, nchan, T, 2, mode, M, coeffs=h, window=(1 if mode == PFB else 0), splits=splits)
+    r, rd = oracle_run(raw, nchan, T, 2, mode, M, coeffs=h, window=(1 if mode == PFB else 0))
+    assert gd == rd == nblk - (T - 1)
+    assert len(g) == len(r) == 2
+    for a, b in zip(g, r):
+        compare(a, b, f"fused N={nchan} mode={mode}")
+        check_stokes_invariants(a)
+
+
+@pytest.mark.parametrize("nchan,mode,nspec,M", [(1024, PFB, 5200, 700), (2048, PFB, 2900, 1000),
+                                                (8192, PFB, 700, 97), (8192, FFT, 700, 256),
+                                                (32768, FFT, 200, 64), (65536, PFB, 130, 50)])
+def test_parity_fused_kernel_ring_wraps(nchan, mode, nspec, M):
+    """Streams longer than the L2-resident Z ring: every ring slot is reused, producers wait for
+    consumers and back; several accumulation windows per call and a partial one left at the end."""
+    T = 8 if mode == PFB else 1
+    nblk = nspec + T - 1
+    raw = synth.dual_pol_stream(400 + nchan // 1024 + mode, nblk * nchan, [synth.F_CFG1])
+    w = 1 if mode == PFB else 0
+    g, gd = gpu_run(raw, nchan, T, 2, mode, M, window=w, splits=[nchan * (nblk - 40), nchan * 40], ring=16)
+    r, rd = oracle_run(raw, nchan, T, 2, mode, M, window=w)
+    assert gd == rd == nspec
+    assert len(g) == len(r) == nspec // M
+    for a, b in zip(g, r):
+        compare(a, b, f"fused ring N={nchan} mode={mode}")
+
+
 @pytest.mark.parametrize("nchan", [131072, 262144, 524288])
 def test_parity_largest_channel_counts(nchan):
     T, M = 8, 2
