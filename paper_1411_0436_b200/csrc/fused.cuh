@@ -15,8 +15,9 @@
 //     added to the HBM accumulator only at accumulation-window boundaries;
 //   * thread 0 of every CTA is its scheduler: run my next B job if its spectra are complete in the
 //     ring, else claim the next A task if the ring has room, else sleep.  Nothing ever blocks inside
-//     a task, dependencies only point to earlier groups, and the grid is launched cooperatively at
-//     exactly the resident size, so the scheme cannot deadlock.
+//     a task, dependencies only point to earlier groups, and the grid is exactly the number of CTAs the
+//     SMs hold at once (registers, shared memory and TMEM columns all sized for it), so the scheme
+//     cannot deadlock.
 // Four-step indexing: n = N2*n1 + n2, k = k1 + 16*k2.
 #pragma once
 #include "engine.cuh"
@@ -38,6 +39,7 @@ struct FusedParams {
     int GS;                // spectra per group (multiple of the A phase length R)
     int RING;              // groups in the Z ring
     int TPG;               // A tasks (column tiles) per group = N2 / 16
+    unsigned long long* dbg;  // optional per-CTA counters (SPEC_FUSED_DEBUG): 8 words per CTA
     unsigned* flags;       // [0] next A task, [1 .. RING] a_done, [1+RING .. 2*RING] b_done (zeroed per launch)
 };
 
@@ -197,11 +199,14 @@ k_fused(const FusedParams p) {
 
     long long bi = 0;      // my next B job (kept by every thread)
     // scheduler state (thread 0)
-    long long ready_g = -1;
+    long long ready_g = -1;   // a group known to be complete in the ring
+    long long freed_g = -1;   // a group known to be fully consumed
+    long long pend_a = -1;    // claimed A task waiting for its ring slot
     bool a_exhausted = false;
     const long long ngroups = (p.nspec + p.GS - 1) / p.GS;
     const long long natasks = ngroups * p.TPG;
 
+    unsigned long long d_idle = 0, d_na = 0, d_nb = 0, d_ta = 0, d_tb = 0, d_ti = 0, d_t0 = clock64(), d_last = d_t0;
     for (int it = 0;; it++) {
         int* ctl = s_ctl[it & 1];
         if (tid == 0) {
@@ -220,24 +225,37 @@ k_fused(const FusedParams p) {
                     type = 1;
                 }
             }
-            if (type == 0 && !a_exhausted) {
-                const unsigned a = ld_relaxed_u32(a_next);
-                if ((long long)a >= natasks) a_exhausted = true;
-                else {
-                    const long long g = a / p.TPG;
-                    const bool room = (g < p.RING) ||
-                        ld_acquire_u32(b_done + g % p.RING) >= (unsigned)((g / p.RING) * p.GS * 16);
-                    if (room && atomicCAS(a_next, a, a + 1) == a) { type = 2; atask = a; }
+            if (type == 0) {
+                // claim the next A task unconditionally (a failed compare-and-swap would serialise the
+                // whole grid), then hold it until its ring slot is free; meanwhile keep serving B jobs
+                if (pend_a < 0 && !a_exhausted) {
+                    const unsigned a = atomicAdd(a_next, 1u);
+                    if ((long long)a >= natasks) a_exhausted = true;
+                    else pend_a = a;
+                }
+                if (pend_a >= 0) {
+                    const long long g = pend_a / p.TPG;
+                    if (g < p.RING || g - p.RING <= freed_g ||
+                        ld_acquire_u32(b_done + g % p.RING) >= (unsigned)((g / p.RING) * p.GS * 16)) {
+                        if (g >= p.RING) freed_g = g - p.RING;
+                        type = 2;
+                        atask = pend_a;
+                        pend_a = -1;
+                    }
                 }
             }
-            if (type == 0 && bi >= nbj && a_exhausted) type = 3;
+            if (type == 0 && bi >= nbj && a_exhausted && pend_a < 0) type = 3;
             ctl[0] = type;
             ctl[1] = (int)atask;
         }
         __syncthreads();
         const int type = ctl[0];
         if (type == 3) break;
-        if (type == 0) { __nanosleep(500); continue; }
+        if (type == 0) {
+            __nanosleep(100);
+            if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_ti += c - d_last; d_last = c; d_idle++; }
+            continue;
+        }
         if (type == 2) {
             const long long a = ctl[1];
             const long long g = a / p.TPG;
@@ -246,6 +264,7 @@ k_fused(const FusedParams p) {
                 __threadfence();
                 atomicAdd(a_done + g % p.RING, 1u);
             }
+            if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_ta += c - d_last; d_last = c; d_na++; }
             continue;
         }
         // ---------------- B job bi
@@ -319,6 +338,11 @@ k_fused(const FusedParams p) {
             }
         }
         // the scheduler's barrier at the top of the next iteration also protects the exchange buffer
+        if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_tb += c - d_last; d_last = c; d_nb++; }
+    }
+    if (p.dbg && tid == 0) {
+        unsigned long long* d = p.dbg + (size_t)blockIdx.x * 8;
+        d[0] = d_idle; d[1] = d_na; d[2] = d_nb; d[3] = d_ti; d[4] = d_ta; d[5] = d_tb; d[6] = clock64() - d_t0; d[7] = d_t0;
     }
     if (wcur >= 0) sink.flush(st, row, t, wcur);
     tmem_free_cta<TCOLS>(tmem_base);

@@ -253,6 +253,9 @@ __global__ void __launch_bounds__(1024, 1) k_fp32_peak(float* out, int iters, fl
 template <class K>
 static int prep_smem(K kern, size_t bytes) {
     if (bytes > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+    // ask for the largest shared-memory carve-out: the default heuristic sized it for one or two CTAs
+    // per SM and capped the occupancy of these kernels below their register limit
+    if (bytes > 0) CK(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     return 0;
 }
 static inline int cdiv(long long a, long long b) { return (int)((a + b - 1) / b); }
@@ -456,10 +459,12 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     if (query) {
         int rc = prep_smem(kern, smem);
         if (rc) return rc;
-        int per_sm = 0;
-        CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, NT, smem));
-        if (per_sm < 1) return SPEC_ERR_CUDA;
-        if (per_sm > 512 / NT) per_sm = 512 / NT;   // tensor memory: 64 (NT=128) / 128 (NT=256) columns per CTA
+        // resident CTAs per SM: 128 registers x 512 threads fill the register file, 4 x 64 (2 x 128) TMEM
+        // columns and 4 x 33 KB of shared memory fit.  The occupancy API cannot be asked: it reports 1
+        // for any kernel that contains tcgen05.alloc (measured: 4 such CTAs of 128 threads do share an
+        // SM), which also rules out cudaLaunchCooperativeKernel for a grid of this size.
+        int per_sm = 512 / NT;
+        if (const char* e = getenv("SPEC_FUSED_CTAS")) { const int v = atoi(e); if (v >= 1 && v <= per_sm) per_sm = v; }
         s->fgrid = per_sm * s->numSM;
         return 0;
     }
@@ -468,11 +473,32 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     p.ring = s->d_ring; p.acc_stride = acc_floats(s); p.nring = s->nring;
     p.N = s->N; p.N2 = s->N2; p.nspec = nspec; p.c0 = c0; p.M = s->M;
     p.GS = s->fGS; p.RING = s->fRING; p.TPG = s->N2 / 16; p.flags = s->d_flags;
+    p.dbg = nullptr;
+    static unsigned long long* dbg_buf = nullptr;
+    const bool dbg = getenv("SPEC_FUSED_DEBUG") != nullptr;
+    if (dbg) {
+        if (!dbg_buf) CK(cudaMalloc(&dbg_buf, (size_t)4096 * 8 * sizeof(unsigned long long)));
+        p.dbg = dbg_buf;
+    }
     CK(cudaMemsetAsync(s->d_flags, 0, (size_t)(1 + 2 * s->fRING) * sizeof(unsigned), st));
-    void* args[] = {&p};
     {
         ProfScope ps(s, 0, st);
-        CK(cudaLaunchCooperativeKernel((void*)kern, dim3(s->fgrid), dim3(NT), args, smem, st));
+        kern<<<dim3(s->fgrid), NT, smem, st>>>(p);
+    }
+    CK(cudaGetLastError());
+    if (dbg) {
+        CK(cudaStreamSynchronize(st));
+        std::vector<unsigned long long> h((size_t)s->fgrid * 8);
+        CK(cudaMemcpy(h.data(), dbg_buf, h.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+        unsigned long long sum[7] = {0, 0, 0, 0, 0, 0, 0}, tmax = 0;
+        for (int c = 0; c < s->fgrid; c++) {
+            for (int k = 0; k < 7; k++) sum[k] += h[(size_t)c * 8 + k];
+            if (h[(size_t)c * 8 + 6] > tmax) tmax = h[(size_t)c * 8 + 6];
+        }
+        fprintf(stderr, "[fused N=%d nspec=%lld grid=%d GS=%d RING=%d] idle_iters=%llu A=%llu B=%llu  cycles/CTA: idle=%llu A=%llu (%.0f/task) B=%llu (%.0f/job) total=%llu max=%llu\n",
+                s->N, nspec, s->fgrid, s->fGS, s->fRING, sum[0], sum[1], sum[2], sum[3] / s->fgrid, sum[4] / s->fgrid,
+                sum[1] ? (double)sum[4] / sum[1] : 0.0, sum[5] / s->fgrid, sum[2] ? (double)sum[5] / sum[2] : 0.0,
+                sum[6] / s->fgrid, tmax);
     }
     return 0;
 }
