@@ -27,20 +27,23 @@ namespace spk {
 struct FusedParams {
     InputView view;        // history ++ input; spectrum j of this launch uses blocks j .. j+T-1
     const float* h;        // T*N coefficients (PFB)
-    float4* Z;             // ring: RS spectra of N float4 (Xre, Yre, Xim, Yim), [spectrum][k1][n2]
+    float4* Z;             // ring: RING*GS spectra of N float4 (Xre, Yre, Xim, Yim), [spectrum][k1][n2]
     const float2* twN;     // W_N^e
     const float2* twL;     // engine stage tables of the N2-point plan
     float* ring;           // accumulator ring (SinkStokesTmem)
     size_t acc_stride;
     int nring;
     int N, N2;
-    long long nspec;       // spectra in this launch
+    int nspec;             // spectra in this launch
     long long c0, M;       // spectra before this launch / per accumulation window
-    int GS;                // spectra per group (multiple of the A phase length R)
+    int lgGS;              // log2 of the spectra per group (a multiple of the A phase length)
     int RING;              // groups in the Z ring
-    int TPG;               // A tasks (column tiles) per group = N2 / 16
+    int lgTPG;             // log2 of the A tasks (column tiles of 16) per group, TPG = N2 / 16
+    int depth;             // producers run at most this many groups ahead of a CTA's own consumer position
+    unsigned* a_next;      // next unclaimed A task            } zeroed before every launch;
+    unsigned* a_done;      // [group] finished A tasks          } one counter per GROUP of the launch,
+    unsigned* b_done;      // [group] consumed rows (of GS*16)  } so no epochs and no divisions
     unsigned long long* dbg;  // optional per-CTA counters (SPEC_FUSED_DEBUG): 8 words per CTA
-    unsigned* flags;       // [0] next A task, [1 .. RING] a_done, [1+RING .. 2*RING] b_done (zeroed per launch)
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
@@ -48,28 +51,84 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+// relaxed counter read: the value may be consumed much later (the scheduler prefetches its polls);
+// ordering against the Z traffic comes from the CTA barrier between the poll and the loads (Z is
+// read with ld.global.cg, so no stale L1 line can be hit) -- an acquire load would invalidate the
+// whole L1 of the SM (CCTL.IVALL) on every poll
 __device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned* p) {
     unsigned v;
     asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ unsigned atom_add_relaxed_u32(unsigned* p, unsigned v) {
+    unsigned r;
+    asm volatile("atom.relaxed.gpu.global.add.u32 %0, [%1], %2;" : "=r"(r) : "l"(p), "r"(v) : "memory");
+    return r;
+}
+__device__ __forceinline__ void red_release_u32(unsigned* p, unsigned v) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 
 // ---------------------------------------------------------------- A task
 // C = 16 adjacent columns n2 (all 16 rows n1: 256 filter branches), the GS spectra of one group,
-// R = NT/16 spectra per phase.  FIR phase: each thread owns 16/R*... branches and slides an 8-sample
-// register window over R+7 blocks; FFT phase: each thread owns one (spectrum, column) pair.
-template <int NT, int MODE_PFB>
-__device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, long long g, int tile) {
-    constexpr int C = 16, R = NT / C, T = 8;
-    constexpr int BPT = 16 * C / NT;  // branches per thread in the FIR phase
+// R = NT/16 spectra per phase.  FIR phase: each thread owns 256/NT branches and slides an 8-sample
+// register window over R+7 blocks (every raw sample of the phase is unpacked once); FFT phase: each
+// thread owns one (spectrum, column) pair.  N is a compile-time constant, so every load and store of
+// a phase is one base register plus an immediate offset.
+template <int NT, int N2, bool RAGGED>
+__device__ __forceinline__ void fused_fir_phase(const FusedParams& p, float4* ysm, const float (&hc)[256 / NT][8],
+                                                const int (&nbr)[256 / NT], int mg, int j0, int nsp) {
+    constexpr int C = 16, R = NT / C, T = 8, N = 16 * N2, BPT = 256 / NT;
     const int tid = threadIdx.x;
-    const int N = p.N, N2 = p.N2;
+    const int qmax = nsp - 1 - j0 + (T - 1);  // last valid block of this phase (ragged tail only)
+    uint32_t raw[BPT][R + T - 1];
+    const bool in_input = (mg + j0 >= p.view.nhist);
+#pragma unroll
+    for (int i = 0; i < BPT; i++) {
+        if (in_input) {
+            const uint32_t* base = (const uint32_t*)p.view.in + (size_t)(mg + j0 - p.view.nhist) * N + nbr[i];
+#pragma unroll
+            for (int q = 0; q < R + T - 1; q++)
+                raw[i][q] = RAGGED ? __ldg(base + (size_t)(q < qmax ? q : qmax) * N) : __ldg(base + q * N);
+        } else {
+#pragma unroll
+            for (int q = 0; q < R + T - 1; q++)
+                raw[i][q] = fetch_raw<2>(p.view, mg + j0 + ((!RAGGED || q < qmax) ? q : qmax), nbr[i], N);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < BPT; i++) {
+        const int beta = tid + NT * i;
+        const int n1 = beta / C, c = beta % C;
+        cpx x[T];
+#pragma unroll
+        for (int t = 0; t < T - 1; t++) x[t] = unpack_cpx<2>(raw[i][t]);
+#pragma unroll
+        for (int r = 0; r < R; r++) {
+            x[(r + T - 1) % T] = unpack_cpx<2>(raw[i][r + T - 1]);
+            u64 re = 0ull, im = 0ull;
+#pragma unroll
+            for (int t = 0; t < T; t++) {
+                re = fma2(x[(r + t) % T].re, bc(hc[i][t]), re);
+                im = fma2(x[(r + t) % T].im, bc(hc[i][t]), im);
+            }
+            ysm[(r * 16 + n1) * C + c] = cpx_to_f4({re, im});
+        }
+    }
+}
+
+template <int NT, int MODE_PFB, int N2>
+__device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, int g, int tile) {
+    constexpr int C = 16, R = NT / C, T = 8, N = 16 * N2;
+    constexpr int BPT = 256 / NT;  // branches per thread in the FIR phase
+    const int tid = threadIdx.x;
     const int n2_0 = tile * C;
-    const long long mg = g * p.GS;                                    // first spectrum of the group
-    const int nsp = (int)((p.nspec - mg < p.GS) ? p.nspec - mg : p.GS);  // valid spectra in it
+    const int GS = 1 << p.lgGS;
+    const int mg = g << p.lgGS;                                   // first spectrum of the group
+    const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;      // valid spectra in it
     const int fr = tid / C, fc = tid % C;
     const int n2 = n2_0 + fc;
-    float4* const zg = p.Z + (size_t)((mg % ((long long)p.RING * p.GS))) * N + n2;
+    float4* const zg = p.Z + ((size_t)((unsigned)g % (unsigned)p.RING) << p.lgGS) * N + n2;
 
     float2 tw[16];
 #pragma unroll
@@ -83,44 +142,11 @@ __device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, 
             const int beta = tid + NT * i;
             nbr[i] = (beta / C) * N2 + n2_0 + (beta % C);
 #pragma unroll
-            for (int t = 0; t < T; t++) hc[i][t] = __ldg(p.h + (size_t)t * N + nbr[i]);
+            for (int t = 0; t < T; t++) hc[i][t] = __ldg(p.h + t * N + nbr[i]);
         }
         for (int j0 = 0; j0 < nsp; j0 += R) {
-            // ---------------- FIR phase: all raw words first (one L2 latency per phase)
-            const int qmax = nsp - 1 - j0 + (T - 1);  // last valid block of this phase (ragged tail)
-            uint32_t raw[BPT][R + T - 1];
-            const bool in_input = (mg + j0 >= p.view.nhist);
-#pragma unroll
-            for (int i = 0; i < BPT; i++) {
-                if (in_input) {
-                    const uint32_t* base = (const uint32_t*)p.view.in + (size_t)(mg + j0 - p.view.nhist) * N + nbr[i];
-#pragma unroll
-                    for (int q = 0; q < R + T - 1; q++) raw[i][q] = __ldg(base + (size_t)(q < qmax ? q : qmax) * N);
-                } else {
-#pragma unroll
-                    for (int q = 0; q < R + T - 1; q++)
-                        raw[i][q] = fetch_raw<2>(p.view, mg + j0 + (q < qmax ? q : qmax), nbr[i], N);
-                }
-            }
-#pragma unroll
-            for (int i = 0; i < BPT; i++) {
-                const int beta = tid + NT * i;
-                const int n1 = beta / C, c = beta % C;
-                cpx x[T];
-#pragma unroll
-                for (int t = 0; t < T - 1; t++) x[t] = unpack_cpx<2>(raw[i][t]);
-#pragma unroll
-                for (int r = 0; r < R; r++) {
-                    x[(r + T - 1) % T] = unpack_cpx<2>(raw[i][r + T - 1]);
-                    u64 re = 0ull, im = 0ull;
-#pragma unroll
-                    for (int t = 0; t < T; t++) {
-                        re = fma2(x[(r + t) % T].re, bc(hc[i][t]), re);
-                        im = fma2(x[(r + t) % T].im, bc(hc[i][t]), im);
-                    }
-                    ysm[(r * 16 + n1) * C + c] = cpx_to_f4({re, im});
-                }
-            }
+            if (j0 + R <= nsp) fused_fir_phase<NT, N2, false>(p, ysm, hc, nbr, mg, j0, nsp);
+            else fused_fir_phase<NT, N2, true>(p, ysm, hc, nbr, mg, j0, nsp);
             __syncthreads();
             // ---------------- column FFT phase
             if (j0 + fr < nsp) {
@@ -131,7 +157,7 @@ __device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, 
                 float4* zp = zg + (size_t)(j0 + fr) * N;
                 zp[0] = cpx_to_f4(v[0]);
 #pragma unroll
-                for (int k = 1; k < 16; k++) zp[(size_t)k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
+                for (int k = 1; k < 16; k++) zp[k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
             }
             __syncthreads();
         }
@@ -143,7 +169,7 @@ __device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, 
                 const uint32_t* base = (const uint32_t*)p.view.in + (size_t)(mg + j0 + fr) * N + n2;
                 uint32_t raw[16];
 #pragma unroll
-                for (int n1 = 0; n1 < 16; n1++) raw[n1] = __ldg(base + (size_t)n1 * N2);
+                for (int n1 = 0; n1 < 16; n1++) raw[n1] = __ldg(base + n1 * N2);
                 cpx v[16];
 #pragma unroll
                 for (int n1 = 0; n1 < 16; n1++) v[n1] = unpack_cpx<2>(raw[n1]);
@@ -151,7 +177,7 @@ __device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, 
                 float4* zp = zg + (size_t)(j0 + fr) * N;
                 zp[0] = cpx_to_f4(v[0]);
 #pragma unroll
-                for (int k = 1; k < 16; k++) zp[(size_t)k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
+                for (int k = 1; k < 16; k++) zp[k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
             }
         }
         __syncthreads();
@@ -175,18 +201,22 @@ k_fused(const FusedParams p) {
 
     const int tid = threadIdx.x;
     const int slot = tid / NTS, t = tid % NTS;
-    unsigned* const a_next = p.flags;
-    unsigned* const a_done = p.flags + 1;
-    unsigned* const b_done = p.flags + 1 + p.RING;
+    const int GS = 1 << p.lgGS;
+    const int RS = p.RING << p.lgGS;                // spectra in the Z ring
 
-    // B ownership: row group rg of every (y + i*ny)-th job
+    // B ownership: row group rg of the jobs y, y+ny, y+2ny, ...  (job j = spectra j*SPJ .. j*SPJ+SPJ-1)
     const int rg = blockIdx.x % RGN;
     const int y = blockIdx.x / RGN;
     const int ny = gridDim.x / RGN;
-    const long long njobs_all = (p.nspec + SPJ - 1) / SPJ;
-    const long long nbj = (y < ny && y < njobs_all) ? (njobs_all - y + ny - 1) / ny : 0;  // my B jobs
+    const int njobs_all = (p.nspec + SPJ - 1) / SPJ;
+    const int nbj = (y < ny && y < njobs_all) ? (njobs_all - y + ny - 1) / ny : 0;  // my B jobs
     const int row = (G >= 16) ? (slot % 16) : (rg * G + slot);
-    const int sub = (G >= 16) ? (slot / 16) : 0;    // spectrum of the job this slot works on
+    const int sub = (G >= 16) ? (slot / 16) : 0;    // which spectrum of the job this slot works on
+    const int mstride = ny * SPJ;
+    const int zstride = mstride % RS;
+    int bi = 0;                                     // my next B job (kept by every thread)
+    int m = y * SPJ + sub;                          // its spectrum for this slot
+    int zpos = m % RS;                              // ring position of that spectrum
 
     auto addr = [&](int q) -> int { return slot * L + (q ^ ((q / 16) & 7)); };
 
@@ -195,90 +225,121 @@ k_fused(const FusedParams p) {
     SinkStokesTmem::State st;
     sink.init(st, tmem_base);
     sink.begin(st);
-    long long wcur = -1;   // accumulation window the TMEM sums belong to (-1: none yet)
+    long long wcur = -1;       // accumulation window the TMEM sums belong to (-1: none yet)
+    long long nextb = 0;       // first spectrum (of this launch) that no longer belongs to window wcur
 
-    long long bi = 0;      // my next B job (kept by every thread)
-    // scheduler state (thread 0)
-    long long ready_g = -1;   // a group known to be complete in the ring
-    long long freed_g = -1;   // a group known to be fully consumed
-    long long pend_a = -1;    // claimed A task waiting for its ring slot
-    bool a_exhausted = false;
-    const long long ngroups = (p.nspec + p.GS - 1) / p.GS;
-    const long long natasks = ngroups * p.TPG;
+    // ---- scheduler state (thread 0).  Polls are PREFETCHED: the counter a decision will need is
+    // loaded right after the previous decision and only looked at one task later, so the L2 round
+    // trip never sits between two tasks; a stale value can only under-report (counters grow).
+    const int ngroups = (p.nspec + GS - 1) >> p.lgGS;
+    const int natasks = ngroups << p.lgTPG;
+    const unsigned TPG = 1u << p.lgTPG;
+    const unsigned rows_full = (unsigned)GS * 16u;
+    int ready_g = -1;          // newest group known to be complete in the ring
+    int freed_g = -1;          // newest group known to be fully consumed (consumption is monotone)
+    int pend_a = -1;           // claimed A task not yet run
+    bool a_exhausted = false, claim_inflight = false;
+    unsigned claim_val = 0;    // async result of the claim
+    unsigned pf_b = 0, pf_r = 0;   // prefetched a_done[pf_bg] / b_done[pf_rg]
+    int pf_bg = -1, pf_rg = -1;
+    auto group_of_job = [&](int j) -> int {
+        int s1 = (y + j * ny) * SPJ + SPJ - 1;
+        if (s1 > p.nspec - 1) s1 = p.nspec - 1;
+        return s1 >> p.lgGS;
+    };
 
+#ifdef SPEC_FUSED_DEBUG_COUNTERS
     unsigned long long d_idle = 0, d_na = 0, d_nb = 0, d_ta = 0, d_tb = 0, d_ti = 0, d_t0 = clock64(), d_last = d_t0;
+#define FDBG(x) x
+#else
+#define FDBG(x)
+#endif
     for (int it = 0;; it++) {
         int* ctl = s_ctl[it & 1];
         if (tid == 0) {
-            int type = 0;  // 0 idle, 1 B job, 2 A task, 3 exit
-            long long atask = 0;
-            if (bi < nbj) {
-                const long long s0 = (y + bi * ny) * SPJ;
-                long long s1 = s0 + SPJ - 1;
-                if (s1 > p.nspec - 1) s1 = p.nspec - 1;
-                const long long g = s1 / p.GS;
-                if (g <= ready_g) type = 1;
-                else if (ld_acquire_u32(a_done + g % p.RING) >= (unsigned)((g / p.RING + 1) * p.TPG)) {
-                    // groups complete in any order, but my jobs ask about non-decreasing g, and a group
-                    // can only be overwritten after I have consumed my rows of it
-                    ready_g = g;
-                    type = 1;
-                }
+            if (claim_inflight) {
+                claim_inflight = false;
+                if ((int)claim_val >= natasks || (int)claim_val < 0) a_exhausted = true;
+                else pend_a = (int)claim_val;
             }
-            if (type == 0) {
-                // claim the next A task unconditionally (a failed compare-and-swap would serialise the
-                // whole grid), then hold it until its ring slot is free; meanwhile keep serving B jobs
-                if (pend_a < 0 && !a_exhausted) {
-                    const unsigned a = atomicAdd(a_next, 1u);
-                    if ((long long)a >= natasks) a_exhausted = true;
-                    else pend_a = a;
-                }
-                if (pend_a >= 0) {
-                    const long long g = pend_a / p.TPG;
-                    if (g < p.RING || g - p.RING <= freed_g ||
-                        ld_acquire_u32(b_done + g % p.RING) >= (unsigned)((g / p.RING) * p.GS * 16)) {
-                        if (g >= p.RING) freed_g = g - p.RING;
-                        type = 2;
-                        atask = pend_a;
-                        pend_a = -1;
+            if (pf_bg >= 0 && pf_b >= TPG && pf_bg > ready_g) ready_g = pf_bg;
+            if (pf_rg >= 0 && pf_r >= rows_full && pf_rg > freed_g) freed_g = pf_rg;
+            int type = 0;  // 0 idle, 1 B job, 2 A task, 3 exit
+            for (int attempt = 0; attempt < 2 && type == 0; attempt++) {
+                const bool b_avail = bi < nbj;
+                const int gB = b_avail ? group_of_job(bi) : 0x3fffffff;
+                const bool b_ready = b_avail && gB == ready_g;
+                const int gA = (pend_a >= 0) ? (pend_a >> p.lgTPG) : -1;
+                const bool a_room = pend_a >= 0 && (gA < p.RING || gA - p.RING <= freed_g);
+                if (a_room && (!b_ready || gA - gB < p.depth)) type = 2;
+                else if (b_ready) type = 1;
+                else if (attempt == 0) {
+                    // slow path: nothing known to be runnable -> fresh polls, claim if nothing is held
+                    if (b_avail && ld_relaxed_u32(p.a_done + gB) >= TPG) ready_g = gB;
+                    if (pend_a < 0 && !a_exhausted) {
+                        const unsigned a = atom_add_relaxed_u32(p.a_next, 1u);
+                        if ((int)a >= natasks || (int)a < 0) a_exhausted = true;
+                        else pend_a = (int)a;
+                    }
+                    if (pend_a >= 0) {
+                        const int g2 = (pend_a >> p.lgTPG) - p.RING;
+                        if (g2 >= 0 && g2 > freed_g && ld_relaxed_u32(p.b_done + g2) >= rows_full) freed_g = g2;
                     }
                 }
             }
             if (type == 0 && bi >= nbj && a_exhausted && pend_a < 0) type = 3;
             ctl[0] = type;
-            ctl[1] = (int)atask;
+            ctl[1] = pend_a;
+            // prefetch what the next decision needs
+            const int nb = bi + (type == 1 ? 1 : 0);
+            pf_bg = -1;
+            if (nb < nbj) {
+                pf_bg = group_of_job(nb);
+                if (pf_bg <= ready_g) pf_bg = -1;
+                else pf_b = ld_relaxed_u32(p.a_done + pf_bg);
+            }
+            if (type == 2) {
+                const int gA = pend_a >> p.lgTPG;
+                pend_a = -1;
+                if (!a_exhausted) {
+                    claim_val = atom_add_relaxed_u32(p.a_next, 1u);
+                    claim_inflight = true;
+                }
+                // the next claim will be about one grid's worth of tasks further on
+                pf_rg = gA + ((int)gridDim.x >> p.lgTPG) + 1 - p.RING;
+                if (pf_rg > ngroups - 1 - p.RING) pf_rg = ngroups - 1 - p.RING;
+            } else if (pend_a >= 0) {
+                pf_rg = (pend_a >> p.lgTPG) - p.RING;
+            } else {
+                pf_rg = -1;
+            }
+            if (pf_rg >= 0 && pf_rg > freed_g) pf_r = ld_relaxed_u32(p.b_done + pf_rg);
+            else pf_rg = -1;
         }
         __syncthreads();
         const int type = ctl[0];
         if (type == 3) break;
         if (type == 0) {
             __nanosleep(100);
-            if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_ti += c - d_last; d_last = c; d_idle++; }
+            FDBG(if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_ti += c - d_last; d_last = c; d_idle++; })
             continue;
         }
         if (type == 2) {
-            const long long a = ctl[1];
-            const long long g = a / p.TPG;
-            fused_task_A<NT, MODE_PFB>(p, smem, g, (int)(a % p.TPG));   // ends with a __syncthreads
-            if (tid == 0) {
-                __threadfence();
-                atomicAdd(a_done + g % p.RING, 1u);
-            }
-            if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_ta += c - d_last; d_last = c; d_na++; }
+            const int a = ctl[1];
+            const int g = a >> p.lgTPG;
+            fused_task_A<NT, MODE_PFB, L>(p, smem, g, a & ((1 << p.lgTPG) - 1));   // ends with a __syncthreads
+            if (tid == 0) red_release_u32(p.a_done + g, 1u);   // all Z stores of the CTA are ordered before it
+            FDBG(if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_ta += c - d_last; d_last = c; d_na++; })
             continue;
         }
-        // ---------------- B job bi
-        const long long s0 = (y + bi * ny) * SPJ;
-        const long long m = s0 + sub;
+        // ---------------- B job bi: spectrum m (ring position zpos), row `row`
         const bool active = m < p.nspec;
-        if (active) {
-            const long long w = (p.c0 + m) / p.M;
-            if (w != wcur) {   // warp-uniform: a warp never straddles spectra
-                if (wcur >= 0) { sink.flush(st, row, t, wcur); sink.begin(st); }
-                wcur = w;
-            }
+        if (active && m >= nextb) {   // new accumulation window (warp-uniform: a warp never straddles spectra)
+            if (wcur >= 0) { sink.flush(st, row, t, wcur); sink.begin(st); }
+            wcur = (p.c0 + m) / p.M;
+            nextb = (wcur + 1) * p.M - p.c0;
         }
-        const float4* zrow = p.Z + (size_t)(m % ((long long)p.RING * p.GS)) * p.N + (size_t)row * L;
+        const float4* zrow = p.Z + (size_t)zpos * (16 * L) + row * L;
         // stage a: rows of Z straight from L2 (ld.global.cg: the ring is rewritten by other SMs)
         if (active) {
 #pragma unroll
@@ -297,14 +358,13 @@ k_fused(const FusedParams p) {
             }
         }
         __syncthreads();
-        if (tid == 0) {   // my rows of this job are consumed: let the producers reuse the ring slot
-            long long s1 = s0 + SPJ;
+        if (tid == 0) {   // my rows of this job are consumed: the producers may reuse the ring slot
+            const int s0 = (y + bi * ny) * SPJ;
+            int s1 = s0 + SPJ;
             if (s1 > p.nspec) s1 = p.nspec;
-            const unsigned rows = (G >= 16) ? (unsigned)(16 * (s1 - s0)) : (unsigned)G;
-            __threadfence();
-            atomicAdd(b_done + (s0 / p.GS) % p.RING, rows);
+            // (a job of several spectra never straddles groups: SPJ divides GS)
+            red_release_u32(p.b_done + (s0 >> p.lgGS), (G >= 16) ? (unsigned)(16 * (s1 - s0)) : (unsigned)G);
         }
-        bi++;
         if (active) {
 #pragma unroll
             for (int u = 0; u < 16 / RB; u++) {
@@ -338,13 +398,17 @@ k_fused(const FusedParams p) {
             }
         }
         // the scheduler's barrier at the top of the next iteration also protects the exchange buffer
-        if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_tb += c - d_last; d_last = c; d_nb++; }
-    }
-    if (p.dbg && tid == 0) {
-        unsigned long long* d = p.dbg + (size_t)blockIdx.x * 8;
-        d[0] = d_idle; d[1] = d_na; d[2] = d_nb; d[3] = d_ti; d[4] = d_ta; d[5] = d_tb; d[6] = clock64() - d_t0; d[7] = d_t0;
+        bi++;
+        m += mstride;
+        zpos += zstride;
+        if (zpos >= RS) zpos -= RS;
+        FDBG(if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_tb += c - d_last; d_last = c; d_nb++; })
     }
     if (wcur >= 0) sink.flush(st, row, t, wcur);
+    FDBG(if (p.dbg && tid == 0) {
+        unsigned long long* d = p.dbg + (size_t)blockIdx.x * 8;
+        d[0] = d_idle; d[1] = d_na; d[2] = d_nb; d[3] = d_ti; d[4] = d_ta; d[5] = d_tb; d[6] = clock64() - d_t0; d[7] = d_t0;
+    })
     tmem_free_cta<TCOLS>(tmem_base);
 }
 

@@ -62,8 +62,9 @@ struct spec_ctx {
     int zbatch = 0;
     // fused persistent four-step kernel (fused.cuh)
     bool fused = false;
-    int fgrid = 0, fGS = 0, fRING = 0;
-    unsigned* d_flags = nullptr;
+    int fgrid = 0, fGS = 0, fRING = 0, fdepth = 3;
+    unsigned* d_flags = nullptr;   // [0] next A task, then a_done[fcap], b_done[fcap] (one counter per group of a launch)
+    int fcap = 0;
     float* d_ring = nullptr;     // nring accumulators of S*N floats, position order, [pos][S]
     int nring = 0;
     float* d_stage = nullptr;    // planar read-out staging, S*N
@@ -468,11 +469,23 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         s->fgrid = per_sm * s->numSM;
         return 0;
     }
+    auto ilog2 = [](int v) { int l = 0; while ((1 << l) < v) l++; return l; };
+    const int ngroups = (int)((nspec + s->fGS - 1) / s->fGS);
+    if (ngroups > s->fcap) {   // grow the per-group counters (rare: first call, or a longer call than any before)
+        CK(cudaStreamSynchronize(st));
+        cudaFree(s->d_flags);
+        s->d_flags = nullptr;
+        s->fcap = 0;
+        const int cap = ngroups + ngroups / 2 + 64;
+        CK(cudaMalloc(&s->d_flags, (size_t)(1 + 2 * cap) * sizeof(unsigned)));
+        s->fcap = cap;
+    }
     FusedParams p;
     p.view = view; p.h = s->d_coef; p.Z = s->d_Z; p.twN = s->d_twN; p.twL = s->d_tw2;
     p.ring = s->d_ring; p.acc_stride = acc_floats(s); p.nring = s->nring;
-    p.N = s->N; p.N2 = s->N2; p.nspec = nspec; p.c0 = c0; p.M = s->M;
-    p.GS = s->fGS; p.RING = s->fRING; p.TPG = s->N2 / 16; p.flags = s->d_flags;
+    p.N = s->N; p.N2 = s->N2; p.nspec = (int)nspec; p.c0 = c0; p.M = s->M;
+    p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / 16); p.depth = s->fdepth;
+    p.a_next = s->d_flags; p.a_done = s->d_flags + 1; p.b_done = s->d_flags + 1 + s->fcap;
     p.dbg = nullptr;
     static unsigned long long* dbg_buf = nullptr;
     const bool dbg = getenv("SPEC_FUSED_DEBUG") != nullptr;
@@ -480,7 +493,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         if (!dbg_buf) CK(cudaMalloc(&dbg_buf, (size_t)4096 * 8 * sizeof(unsigned long long)));
         p.dbg = dbg_buf;
     }
-    CK(cudaMemsetAsync(s->d_flags, 0, (size_t)(1 + 2 * s->fRING) * sizeof(unsigned), st));
+    CK(cudaMemsetAsync(s->d_flags, 0, (size_t)(1 + 2 * s->fcap) * sizeof(unsigned), st));
     {
         ProfScope ps(s, 0, st);
         kern<<<dim3(s->fgrid), NT, smem, st>>>(p);
@@ -602,13 +615,13 @@ static int create_impl(spec_ctx* s) {
             if (rc) return rc;
             const int NT = (s->N2 == 4096) ? 256 : 128;
             s->fGS = (s->N2 >= 512) ? 16 : 64;
-            if (const char* e = getenv("SPEC_FUSED_GS")) { const int v = atoi(e); if (v >= 1 && v <= 4096) s->fGS = v; }
+            if (const char* e = getenv("SPEC_FUSED_GS")) { const int v = atoi(e); if (v >= 2 && v <= 4096 && !(v & (v - 1))) s->fGS = v; }
+            if (const char* e = getenv("SPEC_FUSED_DEPTH")) { const int v = atoi(e); if (v >= 1 && v <= 4096) s->fdepth = v; }
             const long long round_spectra = ((long long)s->fgrid * NT * 16 + N - 1) / N;
             long long rs = 2 * round_spectra + 2 * s->fGS;
             s->fRING = (int)((rs + s->fGS - 1) / s->fGS);
             if (const char* e = getenv("SPEC_FUSED_RING")) { const int v = atoi(e); if (v >= 2 && v <= 4096) s->fRING = v; }
             s->zbatch = s->fRING * s->fGS;
-            CK(cudaMalloc(&s->d_flags, (size_t)(1 + 2 * s->fRING) * sizeof(unsigned)));
         }
         CK(cudaMalloc(&s->d_Z, (size_t)s->zbatch * N * sizeof(float4)));
     }
