@@ -228,24 +228,33 @@ k_fused(const FusedParams p) {
     long long wcur = -1;       // accumulation window the TMEM sums belong to (-1: none yet)
     long long nextb = 0;       // first spectrum (of this launch) that no longer belongs to window wcur
 
-    // ---- scheduler state (thread 0).  Polls are PREFETCHED: the counter a decision will need is
-    // loaded right after the previous decision and only looked at one task later, so the L2 round
-    // trip never sits between two tasks; a stale value can only under-report (counters grow).
+    // ---- scheduler (thread 0).  Its whole state lives in SHARED memory (registers are what the FFT
+    // is short of), A tasks are assigned round-robin (task a = blockIdx.x + k*gridDim.x, no atomic
+    // with a return value), and the two counters a decision needs are PREFETCHED: right after a
+    // decision the 16-byte lines holding a_done[group of my next B job] and b_done[group whose ring
+    // slot my next A task overwrites] are copied global -> shared with cp.async.cg (L2, never a stale
+    // L1 line) and only looked at one task later, so no L2 round trip sits between two tasks.  A stale
+    // value can only under-report: the counters grow monotonically.
     const int ngroups = (p.nspec + GS - 1) >> p.lgGS;
     const int natasks = ngroups << p.lgTPG;
     const unsigned TPG = 1u << p.lgTPG;
     const unsigned rows_full = (unsigned)GS * 16u;
-    int ready_g = -1;          // newest group known to be complete in the ring
-    int freed_g = -1;          // newest group known to be fully consumed (consumption is monotone)
-    int pend_a = -1;           // claimed A task not yet run
-    bool a_exhausted = false, claim_inflight = false;
-    unsigned claim_val = 0;    // async result of the claim
-    unsigned pf_b = 0, pf_r = 0;   // prefetched a_done[pf_bg] / b_done[pf_rg]
-    int pf_bg = -1, pf_rg = -1;
+    __shared__ __align__(16) unsigned s_pf[2][4];   // landing zones of the prefetched counter lines
+    __shared__ int s_sch[8];                        // 0 ready_g, 1 freed_g, 2 next A task, 3 pf_bg, 4 pf_rg
+    if (tid == 0) {
+        s_sch[0] = -1;              // newest group known to be complete in the ring
+        s_sch[1] = -1;              // newest group known to be fully consumed (consumption is monotone)
+        s_sch[2] = blockIdx.x;      // my next A task
+        s_sch[3] = -1;              // group whose a_done line is in s_pf[0]
+        s_sch[4] = -1;              // group whose b_done line is in s_pf[1]
+    }
     auto group_of_job = [&](int j) -> int {
         int s1 = (y + j * ny) * SPJ + SPJ - 1;
         if (s1 > p.nspec - 1) s1 = p.nspec - 1;
         return s1 >> p.lgGS;
+    };
+    auto prefetch_line = [&](unsigned* dst, const unsigned* src) {
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
     };
 
 #ifdef SPEC_FUSED_DEBUG_COUNTERS
@@ -257,64 +266,43 @@ k_fused(const FusedParams p) {
     for (int it = 0;; it++) {
         int* ctl = s_ctl[it & 1];
         if (tid == 0) {
-            if (claim_inflight) {
-                claim_inflight = false;
-                if ((int)claim_val >= natasks || (int)claim_val < 0) a_exhausted = true;
-                else pend_a = (int)claim_val;
-            }
-            if (pf_bg >= 0 && pf_b >= TPG && pf_bg > ready_g) ready_g = pf_bg;
-            if (pf_rg >= 0 && pf_r >= rows_full && pf_rg > freed_g) freed_g = pf_rg;
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            int ready_g = s_sch[0], freed_g = s_sch[1];
+            const int a_cur = s_sch[2];
+            const int pf_bg = s_sch[3], pf_rg = s_sch[4];
+            if (pf_bg >= 0 && s_pf[0][pf_bg & 3] >= TPG && pf_bg > ready_g) ready_g = pf_bg;
+            if (pf_rg >= 0 && s_pf[1][pf_rg & 3] >= rows_full && pf_rg > freed_g) freed_g = pf_rg;
+            const bool a_avail = a_cur < natasks;
+            const bool b_avail = bi < nbj;
+            const int gB = b_avail ? group_of_job(bi) : 0x3fffffff;
+            const int gA = a_avail ? (a_cur >> p.lgTPG) : -1;
             int type = 0;  // 0 idle, 1 B job, 2 A task, 3 exit
             for (int attempt = 0; attempt < 2 && type == 0; attempt++) {
-                const bool b_avail = bi < nbj;
-                const int gB = b_avail ? group_of_job(bi) : 0x3fffffff;
                 const bool b_ready = b_avail && gB == ready_g;
-                const int gA = (pend_a >= 0) ? (pend_a >> p.lgTPG) : -1;
-                const bool a_room = pend_a >= 0 && (gA < p.RING || gA - p.RING <= freed_g);
+                const bool a_room = a_avail && (gA < p.RING || gA - p.RING <= freed_g);
                 if (a_room && (!b_ready || gA - gB < p.depth)) type = 2;
                 else if (b_ready) type = 1;
-                else if (attempt == 0) {
-                    // slow path: nothing known to be runnable -> fresh polls, claim if nothing is held
+                else if (attempt == 0) {   // slow path: nothing known to be runnable -> fresh polls
                     if (b_avail && ld_relaxed_u32(p.a_done + gB) >= TPG) ready_g = gB;
-                    if (pend_a < 0 && !a_exhausted) {
-                        const unsigned a = atom_add_relaxed_u32(p.a_next, 1u);
-                        if ((int)a >= natasks || (int)a < 0) a_exhausted = true;
-                        else pend_a = (int)a;
-                    }
-                    if (pend_a >= 0) {
-                        const int g2 = (pend_a >> p.lgTPG) - p.RING;
-                        if (g2 >= 0 && g2 > freed_g && ld_relaxed_u32(p.b_done + g2) >= rows_full) freed_g = g2;
-                    }
+                    if (a_avail && gA >= p.RING && ld_relaxed_u32(p.b_done + gA - p.RING) >= rows_full) freed_g = gA - p.RING;
                 }
             }
-            if (type == 0 && bi >= nbj && a_exhausted && pend_a < 0) type = 3;
+            if (type == 0 && !b_avail && !a_avail) type = 3;
             ctl[0] = type;
-            ctl[1] = pend_a;
+            ctl[1] = a_cur;
             // prefetch what the next decision needs
             const int nb = bi + (type == 1 ? 1 : 0);
-            pf_bg = -1;
+            int nbg = -1;
             if (nb < nbj) {
-                pf_bg = group_of_job(nb);
-                if (pf_bg <= ready_g) pf_bg = -1;
-                else pf_b = ld_relaxed_u32(p.a_done + pf_bg);
+                nbg = group_of_job(nb);
+                if (nbg <= ready_g) nbg = -1;
+                else prefetch_line(s_pf[0], p.a_done + (nbg & ~3));
             }
-            if (type == 2) {
-                const int gA = pend_a >> p.lgTPG;
-                pend_a = -1;
-                if (!a_exhausted) {
-                    claim_val = atom_add_relaxed_u32(p.a_next, 1u);
-                    claim_inflight = true;
-                }
-                // the next claim will be about one grid's worth of tasks further on
-                pf_rg = gA + ((int)gridDim.x >> p.lgTPG) + 1 - p.RING;
-                if (pf_rg > ngroups - 1 - p.RING) pf_rg = ngroups - 1 - p.RING;
-            } else if (pend_a >= 0) {
-                pf_rg = (pend_a >> p.lgTPG) - p.RING;
-            } else {
-                pf_rg = -1;
-            }
-            if (pf_rg >= 0 && pf_rg > freed_g) pf_r = ld_relaxed_u32(p.b_done + pf_rg);
-            else pf_rg = -1;
+            const int na = a_cur + (type == 2 ? (int)gridDim.x : 0);
+            int nrg = (na < natasks) ? (na >> p.lgTPG) - p.RING : -1;
+            if (nrg >= 0 && nrg > freed_g) prefetch_line(s_pf[1], p.b_done + (nrg & ~3));
+            else nrg = -1;
+            s_sch[0] = ready_g; s_sch[1] = freed_g; s_sch[2] = na; s_sch[3] = nbg; s_sch[4] = nrg;
         }
         __syncthreads();
         const int type = ctl[0];

@@ -476,8 +476,8 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         cudaFree(s->d_flags);
         s->d_flags = nullptr;
         s->fcap = 0;
-        const int cap = ngroups + ngroups / 2 + 64;
-        CK(cudaMalloc(&s->d_flags, (size_t)(1 + 2 * cap) * sizeof(unsigned)));
+        const int cap = (ngroups + ngroups / 2 + 64) & ~3;   // counters are prefetched as 16-byte lines
+        CK(cudaMalloc(&s->d_flags, (size_t)(4 + 2 * cap) * sizeof(unsigned)));
         s->fcap = cap;
     }
     FusedParams p;
@@ -485,7 +485,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     p.ring = s->d_ring; p.acc_stride = acc_floats(s); p.nring = s->nring;
     p.N = s->N; p.N2 = s->N2; p.nspec = (int)nspec; p.c0 = c0; p.M = s->M;
     p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / 16); p.depth = s->fdepth;
-    p.a_next = s->d_flags; p.a_done = s->d_flags + 1; p.b_done = s->d_flags + 1 + s->fcap;
+    p.a_next = s->d_flags; p.a_done = s->d_flags + 4; p.b_done = s->d_flags + 4 + s->fcap;
     p.dbg = nullptr;
     static unsigned long long* dbg_buf = nullptr;
     const bool dbg = getenv("SPEC_FUSED_DEBUG") != nullptr;
@@ -493,7 +493,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         if (!dbg_buf) CK(cudaMalloc(&dbg_buf, (size_t)4096 * 8 * sizeof(unsigned long long)));
         p.dbg = dbg_buf;
     }
-    CK(cudaMemsetAsync(s->d_flags, 0, (size_t)(1 + 2 * s->fcap) * sizeof(unsigned), st));
+    CK(cudaMemsetAsync(s->d_flags, 0, (size_t)(4 + 2 * s->fcap) * sizeof(unsigned), st));
     {
         ProfScope ps(s, 0, st);
         kern<<<dim3(s->fgrid), NT, smem, st>>>(p);
