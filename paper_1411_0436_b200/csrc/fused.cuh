@@ -5,19 +5,22 @@
 //            (step 5)
 //
 // The paper runs these as separate kernels around a library FFT, one launch set per FFT invocation
-// (PAPER.md:90-95, :116).  Here every CTA of one resident grid is both producer and consumer:
+// (PAPER.md:90-95, :116).  Here one resident grid holds producers and consumers side by side:
 //   * the intermediate Z is a RING of `RING` groups of `GS` spectra that stays in the 126 MB L2;
-//     monotonic counters (a_done / b_done per ring slot) order producers and consumers, so a whole
-//     spec_process call is one launch however many spectra it holds;
-//   * each CTA owns a fixed set of channels (rows k1 of the four-step split) for an interleaved
-//     subset of the spectra; their four Stokes sums live in TENSOR MEMORY (tcgen05.ld/st), not in
-//     registers, so the FFT runs at 128 registers per thread and four CTAs per SM, and they are
-//     added to the HBM accumulator only at accumulation-window boundaries;
-//   * thread 0 of every CTA is its scheduler: run my next B job if its spectra are complete in the
-//     ring, else claim the next A task if the ring has room, else sleep.  Nothing ever blocks inside
-//     a task, dependencies only point to earlier groups, and the grid is exactly the number of CTAs the
-//     SMs hold at once (registers, shared memory and TMEM columns all sized for it), so the scheme
-//     cannot deadlock.
+//     one monotonic counter pair per group (a_done / b_done) orders producers and consumers, so a
+//     whole spec_process call is one launch however many spectra it holds;
+//   * every SM hosts `na_per_sm` PRODUCER CTAs (A tasks, round-robin over the task list) and the rest
+//     of its CTAs as CONSUMERS (each owns fixed rows k1 of the four-step split for an interleaved
+//     subset of the spectra).  The role comes from the order of arrival on the SM (%smid counter), so
+//     both kinds always share an SM: whichever side is blocked leaves its issue slots to the other,
+//     which balances the two rates without any scheduler;
+//   * the consumers' four Stokes sums live in TENSOR MEMORY (tcgen05.ld/st), not in registers, so
+//     the FFT runs at 128 registers per thread and four CTAs per SM; they are added to the HBM
+//     accumulator only at accumulation-window boundaries;
+//   * a producer waits (thread 0, prefetched poll) only for the ring slot it is about to overwrite, a
+//     consumer only for the group it is about to read; dependencies point to earlier groups only and
+//     the grid is exactly the number of CTAs the SMs hold at once (the register file allows no more
+//     per SM, so every SM gets the same mix), hence no deadlock.
 // Four-step indexing: n = N2*n1 + n2, k = k1 + 16*k2.
 #pragma once
 #include "engine.cuh"
@@ -39,10 +42,10 @@ struct FusedParams {
     int lgGS;              // log2 of the spectra per group (a multiple of the A phase length)
     int RING;              // groups in the Z ring
     int lgTPG;             // log2 of the A tasks (column tiles of 16) per group, TPG = N2 / 16
-    int depth;             // producers run at most this many groups ahead of a CTA's own consumer position
-    unsigned* a_next;      // next unclaimed A task            } zeroed before every launch;
-    unsigned* a_done;      // [group] finished A tasks          } one counter per GROUP of the launch,
-    unsigned* b_done;      // [group] consumed rows (of GS*16)  } so no epochs and no divisions
+    int na_per_sm;         // producer CTAs per SM (the others consume)
+    unsigned* role;        // [0] producer rank counter, [1] consumer rank counter, [2] arrivals, [4 + smid] CTAs seen on that SM
+    unsigned* a_done;      // [group] finished A tasks          } zeroed before every launch; one counter per
+    unsigned* b_done;      // [group] consumed rows (of GS*16)  } GROUP of the launch: no epochs, no divisions
     unsigned long long* dbg;  // optional per-CTA counters (SPEC_FUSED_DEBUG): 8 words per CTA
 };
 
@@ -117,8 +120,11 @@ __device__ __forceinline__ void fused_fir_phase(const FusedParams& p, float4* ys
     }
 }
 
-template <int NT, int MODE_PFB, int N2>
-__device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, int g, int tile) {
+// `wait_room` (called by thread 0 only) returns once the ring slot of group g may be overwritten; it
+// sits in front of the first barrier that precedes a Z store, so the loads and the FIR of the first
+// phase overlap the wait.
+template <int NT, int MODE_PFB, int N2, class WaitRoom>
+__device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, int g, int tile, WaitRoom wait_room) {
     constexpr int C = 16, R = NT / C, T = 8, N = 16 * N2;
     constexpr int BPT = 256 / NT;  // branches per thread in the FIR phase
     const int tid = threadIdx.x;
@@ -147,6 +153,7 @@ __device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, 
         for (int j0 = 0; j0 < nsp; j0 += R) {
             if (j0 + R <= nsp) fused_fir_phase<NT, N2, false>(p, ysm, hc, nbr, mg, j0, nsp);
             else fused_fir_phase<NT, N2, true>(p, ysm, hc, nbr, mg, j0, nsp);
+            if (j0 == 0 && tid == 0) wait_room();
             __syncthreads();
             // ---------------- column FFT phase
             if (j0 + fr < nsp) {
@@ -164,6 +171,8 @@ __device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, 
     } else {
         // direct-FFT mode: no pre-filter, the 16 samples of a column go straight from
         // global memory through the unpack into the butterfly
+        if (tid == 0) wait_room();
+        __syncthreads();
         for (int j0 = 0; j0 < nsp; j0 += R) {
             if (j0 + fr < nsp) {
                 const uint32_t* base = (const uint32_t*)p.view.in + (size_t)(mg + j0 + fr) * N + n2;
@@ -196,130 +205,113 @@ k_fused(const FusedParams p) {
     constexpr int TCOLS = (NT > 128) ? 128 : 64;
     static_assert(NST >= 2 && PL::RLAST == 16 && G * L * 16 == NT * 256, "row plan");
     extern __shared__ float4 smem[];                // G*L float4: B exchange buffer / A FIR hand-off
-    __shared__ int s_ctl[2][4];
+    __shared__ int s_role[2];
     __shared__ uint32_t s_tmem;
+    __shared__ __align__(16) unsigned s_pf[4];      // landing zone of the prefetched counter line
 
     const int tid = threadIdx.x;
-    const int slot = tid / NTS, t = tid % NTS;
     const int GS = 1 << p.lgGS;
-    const int RS = p.RING << p.lgGS;                // spectra in the Z ring
+    const int ngroups = (p.nspec + GS - 1) >> p.lgGS;
+    const unsigned TPG = 1u << p.lgTPG;
+    const unsigned rows_full = (unsigned)GS * 16u;
 
-    // B ownership: row group rg of the jobs y, y+ny, y+2ny, ...  (job j = spectra j*SPJ .. j*SPJ+SPJ-1)
-    const int rg = blockIdx.x % RGN;
-    const int y = blockIdx.x / RGN;
-    const int ny = gridDim.x / RGN;
+    // Every CTA allocates its TMEM columns first, producers included: a CTA of a kernel that contains
+    // tcgen05.alloc holds the SM's allocation permit until it relinquishes it, and (measured) no
+    // further CTA of the grid is started on that SM before then.
+    const uint32_t tmem_base = tmem_alloc_cta<TCOLS>(&s_tmem);
+
+    // role and rank: the first na_per_sm CTAs to arrive on an SM produce, the others consume
+    if (tid == 0) {
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        const unsigned li = atomicAdd(p.role + 4 + smid, 1u);
+        const int is_a = li < (unsigned)p.na_per_sm;
+        s_role[0] = is_a;
+        s_role[1] = (int)atomicAdd(p.role + (is_a ? 0 : 1), 1u);
+        atomicAdd(p.role + 2, 1u);   // arrivals
+    }
+    __syncthreads();
+    // No CTA may leave before every CTA of the grid has arrived: an early exit would free a slot on its
+    // SM, a late CTA would land there as a fifth arrival and the per-SM role split would be off.
+    auto leave = [&]() {
+        if (tid == 0)
+            while (ld_relaxed_u32(p.role + 2) < gridDim.x) __nanosleep(200);
+    };
+    const bool is_a = s_role[0] != 0;
+    const int rank = s_role[1];
+    const int per_sm = 512 / NT;
+    const int nsm = (int)gridDim.x / per_sm;
+    auto prefetch_line = [&](const unsigned* src) {
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(s_pf)), "l"(src) : "memory");
+    };
+
+    if (is_a) {
+        // ================= producer: A tasks rank, rank + NA, ...
+        const int NA = nsm * p.na_per_sm;
+        const int natasks = ngroups << p.lgTPG;
+        for (int a = rank; a < natasks; a += NA) {
+            const int g = a >> p.lgTPG;
+            const int gfree = g - p.RING;     // the group whose ring slot this task overwrites
+            if (tid == 0 && gfree >= 0) prefetch_line(p.b_done + (gfree & ~3));
+            fused_task_A<NT, MODE_PFB, L>(p, smem, g, a & (int)(TPG - 1), [&]() {
+                if (gfree < 0) return;
+                asm volatile("cp.async.wait_all;" ::: "memory");
+                if (*(volatile unsigned*)&s_pf[gfree & 3] >= rows_full) return;
+                while (ld_relaxed_u32(p.b_done + gfree) < rows_full) __nanosleep(200);
+            });   // ends with a __syncthreads
+            if (tid == 0) red_release_u32(p.a_done + g, 1u);   // all Z stores of the CTA are ordered before it
+        }
+        leave();
+        tmem_free_cta<TCOLS>(tmem_base);
+        return;
+    }
+
+    // ================= consumer: row group rg of the jobs y, y+ny, y+2ny, ...  (job j = spectra j*SPJ ..)
+    const int NB = nsm * (per_sm - p.na_per_sm);
+    const int slot = tid / NTS, t = tid % NTS;
+    const int RS = p.RING << p.lgGS;                // spectra in the Z ring
+    const int rg = rank % RGN;
+    const int y = rank / RGN;
+    const int ny = NB / RGN;
     const int njobs_all = (p.nspec + SPJ - 1) / SPJ;
     const int nbj = (y < ny && y < njobs_all) ? (njobs_all - y + ny - 1) / ny : 0;  // my B jobs
     const int row = (G >= 16) ? (slot % 16) : (rg * G + slot);
     const int sub = (G >= 16) ? (slot / 16) : 0;    // which spectrum of the job this slot works on
     const int mstride = ny * SPJ;
     const int zstride = mstride % RS;
-    int bi = 0;                                     // my next B job (kept by every thread)
-    int m = y * SPJ + sub;                          // its spectrum for this slot
-    int zpos = m % RS;                              // ring position of that spectrum
-
+    int m = y * SPJ + sub;                          // spectrum of my next job for this slot
+    int zpos = m % RS;                              // its ring position
     auto addr = [&](int q) -> int { return slot * L + (q ^ ((q / 16) & 7)); };
+    auto group_of_job = [&](int j) -> int {
+        int s1 = (y + j * ny) * SPJ + SPJ - 1;
+        if (s1 > p.nspec - 1) s1 = p.nspec - 1;
+        return s1 >> p.lgGS;
+    };
 
-    const uint32_t tmem_base = tmem_alloc_cta<TCOLS>(&s_tmem);
     SinkStokesTmem sink{p.ring, p.acc_stride, p.nring, L, 1};
     SinkStokesTmem::State st;
     sink.init(st, tmem_base);
     sink.begin(st);
     long long wcur = -1;       // accumulation window the TMEM sums belong to (-1: none yet)
     long long nextb = 0;       // first spectrum (of this launch) that no longer belongs to window wcur
+    int ready_g = -1;          // thread 0: newest group known to be complete
 
-    // ---- scheduler (thread 0).  Its whole state lives in SHARED memory (registers are what the FFT
-    // is short of), A tasks are assigned round-robin (task a = blockIdx.x + k*gridDim.x, no atomic
-    // with a return value), and the two counters a decision needs are PREFETCHED: right after a
-    // decision the 16-byte lines holding a_done[group of my next B job] and b_done[group whose ring
-    // slot my next A task overwrites] are copied global -> shared with cp.async.cg (L2, never a stale
-    // L1 line) and only looked at one task later, so no L2 round trip sits between two tasks.  A stale
-    // value can only under-report: the counters grow monotonically.
-    const int ngroups = (p.nspec + GS - 1) >> p.lgGS;
-    const int natasks = ngroups << p.lgTPG;
-    const unsigned TPG = 1u << p.lgTPG;
-    const unsigned rows_full = (unsigned)GS * 16u;
-    __shared__ __align__(16) unsigned s_pf[2][4];   // landing zones of the prefetched counter lines
-    __shared__ int s_sch[8];                        // 0 ready_g, 1 freed_g, 2 next A task, 3 pf_bg, 4 pf_rg
-    if (tid == 0) {
-        s_sch[0] = -1;              // newest group known to be complete in the ring
-        s_sch[1] = -1;              // newest group known to be fully consumed (consumption is monotone)
-        s_sch[2] = blockIdx.x;      // my next A task
-        s_sch[3] = -1;              // group whose a_done line is in s_pf[0]
-        s_sch[4] = -1;              // group whose b_done line is in s_pf[1]
-    }
-    auto group_of_job = [&](int j) -> int {
-        int s1 = (y + j * ny) * SPJ + SPJ - 1;
-        if (s1 > p.nspec - 1) s1 = p.nspec - 1;
-        return s1 >> p.lgGS;
-    };
-    auto prefetch_line = [&](unsigned* dst, const unsigned* src) {
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
-    };
-
-#ifdef SPEC_FUSED_DEBUG_COUNTERS
-    unsigned long long d_idle = 0, d_na = 0, d_nb = 0, d_ta = 0, d_tb = 0, d_ti = 0, d_t0 = clock64(), d_last = d_t0;
-#define FDBG(x) x
-#else
-#define FDBG(x)
-#endif
-    for (int it = 0;; it++) {
-        int* ctl = s_ctl[it & 1];
+    if (tid == 0 && nbj > 0) prefetch_line(p.a_done + (group_of_job(0) & ~3));
+    for (int bi = 0; bi < nbj; bi++) {
         if (tid == 0) {
-            asm volatile("cp.async.wait_all;" ::: "memory");
-            int ready_g = s_sch[0], freed_g = s_sch[1];
-            const int a_cur = s_sch[2];
-            const int pf_bg = s_sch[3], pf_rg = s_sch[4];
-            if (pf_bg >= 0 && s_pf[0][pf_bg & 3] >= TPG && pf_bg > ready_g) ready_g = pf_bg;
-            if (pf_rg >= 0 && s_pf[1][pf_rg & 3] >= rows_full && pf_rg > freed_g) freed_g = pf_rg;
-            const bool a_avail = a_cur < natasks;
-            const bool b_avail = bi < nbj;
-            const int gB = b_avail ? group_of_job(bi) : 0x3fffffff;
-            const int gA = a_avail ? (a_cur >> p.lgTPG) : -1;
-            int type = 0;  // 0 idle, 1 B job, 2 A task, 3 exit
-            for (int attempt = 0; attempt < 2 && type == 0; attempt++) {
-                const bool b_ready = b_avail && gB == ready_g;
-                const bool a_room = a_avail && (gA < p.RING || gA - p.RING <= freed_g);
-                if (a_room && (!b_ready || gA - gB < p.depth)) type = 2;
-                else if (b_ready) type = 1;
-                else if (attempt == 0) {   // slow path: nothing known to be runnable -> fresh polls
-                    if (b_avail && ld_relaxed_u32(p.a_done + gB) >= TPG) ready_g = gB;
-                    if (a_avail && gA >= p.RING && ld_relaxed_u32(p.b_done + gA - p.RING) >= rows_full) freed_g = gA - p.RING;
-                }
+            const int g = group_of_job(bi);
+            if (g != ready_g) {
+                asm volatile("cp.async.wait_all;" ::: "memory");
+                if (*(volatile unsigned*)&s_pf[g & 3] < TPG)
+                    while (ld_relaxed_u32(p.a_done + g) < TPG) __nanosleep(200);
+                ready_g = g;
             }
-            if (type == 0 && !b_avail && !a_avail) type = 3;
-            ctl[0] = type;
-            ctl[1] = a_cur;
-            // prefetch what the next decision needs
-            const int nb = bi + (type == 1 ? 1 : 0);
-            int nbg = -1;
-            if (nb < nbj) {
-                nbg = group_of_job(nb);
-                if (nbg <= ready_g) nbg = -1;
-                else prefetch_line(s_pf[0], p.a_done + (nbg & ~3));
+            if (bi + 1 < nbj) {
+                const int g1 = group_of_job(bi + 1);
+                if (g1 != ready_g) prefetch_line(p.a_done + (g1 & ~3));
             }
-            const int na = a_cur + (type == 2 ? (int)gridDim.x : 0);
-            int nrg = (na < natasks) ? (na >> p.lgTPG) - p.RING : -1;
-            if (nrg >= 0 && nrg > freed_g) prefetch_line(s_pf[1], p.b_done + (nrg & ~3));
-            else nrg = -1;
-            s_sch[0] = ready_g; s_sch[1] = freed_g; s_sch[2] = na; s_sch[3] = nbg; s_sch[4] = nrg;
         }
-        __syncthreads();
-        const int type = ctl[0];
-        if (type == 3) break;
-        if (type == 0) {
-            __nanosleep(100);
-            FDBG(if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_ti += c - d_last; d_last = c; d_idle++; })
-            continue;
-        }
-        if (type == 2) {
-            const int a = ctl[1];
-            const int g = a >> p.lgTPG;
-            fused_task_A<NT, MODE_PFB, L>(p, smem, g, a & ((1 << p.lgTPG) - 1));   // ends with a __syncthreads
-            if (tid == 0) red_release_u32(p.a_done + g, 1u);   // all Z stores of the CTA are ordered before it
-            FDBG(if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_ta += c - d_last; d_last = c; d_na++; })
-            continue;
-        }
+        __syncthreads();   // publishes "group complete"; also frees the exchange buffer of the previous job
         // ---------------- B job bi: spectrum m (ring position zpos), row `row`
         const bool active = m < p.nspec;
         if (active && m >= nextb) {   // new accumulation window (warp-uniform: a warp never straddles spectra)
@@ -385,18 +377,12 @@ k_fused(const FusedParams p) {
                 sink.put16(st, m, 0, t, 0, 1, v);
             }
         }
-        // the scheduler's barrier at the top of the next iteration also protects the exchange buffer
-        bi++;
         m += mstride;
         zpos += zstride;
         if (zpos >= RS) zpos -= RS;
-        FDBG(if (p.dbg && tid == 0) { const unsigned long long c = clock64(); d_tb += c - d_last; d_last = c; d_nb++; })
     }
     if (wcur >= 0) sink.flush(st, row, t, wcur);
-    FDBG(if (p.dbg && tid == 0) {
-        unsigned long long* d = p.dbg + (size_t)blockIdx.x * 8;
-        d[0] = d_idle; d[1] = d_na; d[2] = d_nb; d[3] = d_ti; d[4] = d_ta; d[5] = d_tb; d[6] = clock64() - d_t0; d[7] = d_t0;
-    })
+    leave();
     tmem_free_cta<TCOLS>(tmem_base);
 }
 

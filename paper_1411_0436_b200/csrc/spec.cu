@@ -8,6 +8,7 @@
 #include <stdio.h>
 #include <stdlib.h>
 #include <string.h>
+#include <time.h>
 
 #include <type_traits>
 #include <vector>
@@ -62,7 +63,7 @@ struct spec_ctx {
     int zbatch = 0;
     // fused persistent four-step kernel (fused.cuh)
     bool fused = false;
-    int fgrid = 0, fGS = 0, fRING = 0, fdepth = 3;
+    int fgrid = 0, fGS = 0, fRING = 0, fna = 2;   // grid, spectra per group, ring groups, producer CTAs per SM
     unsigned* d_flags = nullptr;   // [0] next A task, then a_done[fcap], b_done[fcap] (one counter per group of a launch)
     int fcap = 0;
     float* d_ring = nullptr;     // nring accumulators of S*N floats, position order, [pos][S]
@@ -452,7 +453,8 @@ static int run_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
     return SPEC_ERR_ARG;
 }
 
-// ---- fused persistent four-step kernel (fused.cuh): one cooperative launch per call
+// ---- fused persistent four-step kernel (fused.cuh): one launch per call
+static const int FUSED_ROLE_WORDS = 516;   // 2 rank counters (+2 pad), 512 per-SM arrival counters; keeps the rest 16-byte aligned
 template <class PL, int NT, int MODE_PFB>
 static int fused_do(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
     auto kern = k_fused<PL, NT, MODE_PFB>;
@@ -477,41 +479,42 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         s->d_flags = nullptr;
         s->fcap = 0;
         const int cap = (ngroups + ngroups / 2 + 64) & ~3;   // counters are prefetched as 16-byte lines
-        CK(cudaMalloc(&s->d_flags, (size_t)(4 + 2 * cap) * sizeof(unsigned)));
+        CK(cudaMalloc(&s->d_flags, (size_t)(FUSED_ROLE_WORDS + 2 * cap) * sizeof(unsigned)));
         s->fcap = cap;
     }
     FusedParams p;
     p.view = view; p.h = s->d_coef; p.Z = s->d_Z; p.twN = s->d_twN; p.twL = s->d_tw2;
     p.ring = s->d_ring; p.acc_stride = acc_floats(s); p.nring = s->nring;
     p.N = s->N; p.N2 = s->N2; p.nspec = (int)nspec; p.c0 = c0; p.M = s->M;
-    p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / 16); p.depth = s->fdepth;
-    p.a_next = s->d_flags; p.a_done = s->d_flags + 4; p.b_done = s->d_flags + 4 + s->fcap;
+    p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / 16); p.na_per_sm = s->fna;
+    p.role = s->d_flags; p.a_done = s->d_flags + FUSED_ROLE_WORDS; p.b_done = s->d_flags + FUSED_ROLE_WORDS + s->fcap;
     p.dbg = nullptr;
-    static unsigned long long* dbg_buf = nullptr;
-    const bool dbg = getenv("SPEC_FUSED_DEBUG") != nullptr;
-    if (dbg) {
-        if (!dbg_buf) CK(cudaMalloc(&dbg_buf, (size_t)4096 * 8 * sizeof(unsigned long long)));
-        p.dbg = dbg_buf;
-    }
-    CK(cudaMemsetAsync(s->d_flags, 0, (size_t)(4 + 2 * s->fcap) * sizeof(unsigned), st));
+    CK(cudaMemsetAsync(s->d_flags, 0, (size_t)(FUSED_ROLE_WORDS + 2 * s->fcap) * sizeof(unsigned), st));
     {
         ProfScope ps(s, 0, st);
         kern<<<dim3(s->fgrid), NT, smem, st>>>(p);
     }
     CK(cudaGetLastError());
-    if (dbg) {
-        CK(cudaStreamSynchronize(st));
-        std::vector<unsigned long long> h((size_t)s->fgrid * 8);
-        CK(cudaMemcpy(h.data(), dbg_buf, h.size() * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
-        unsigned long long sum[7] = {0, 0, 0, 0, 0, 0, 0}, tmax = 0;
-        for (int c = 0; c < s->fgrid; c++) {
-            for (int k = 0; k < 7; k++) sum[k] += h[(size_t)c * 8 + k];
-            if (h[(size_t)c * 8 + 6] > tmax) tmax = h[(size_t)c * 8 + 6];
+    if (getenv("SPEC_FUSED_WATCHDOG")) {   // debugging aid: dump the counters if the launch does not finish
+        for (int ms = 0; ms < 3000 && cudaStreamQuery(st) == cudaErrorNotReady; ms++) {
+            struct timespec ts = {0, 1000000};
+            nanosleep(&ts, nullptr);
         }
-        fprintf(stderr, "[fused N=%d nspec=%lld grid=%d GS=%d RING=%d] idle_iters=%llu A=%llu B=%llu  cycles/CTA: idle=%llu A=%llu (%.0f/task) B=%llu (%.0f/job) total=%llu max=%llu\n",
-                s->N, nspec, s->fgrid, s->fGS, s->fRING, sum[0], sum[1], sum[2], sum[3] / s->fgrid, sum[4] / s->fgrid,
-                sum[1] ? (double)sum[4] / sum[1] : 0.0, sum[5] / s->fgrid, sum[2] ? (double)sum[5] / sum[2] : 0.0,
-                sum[6] / s->fgrid, tmax);
+        if (cudaStreamQuery(st) == cudaErrorNotReady) {
+            cudaStream_t side;
+            cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking);
+            std::vector<unsigned> h((size_t)FUSED_ROLE_WORDS + 2 * s->fcap);
+            cudaMemcpyAsync(h.data(), s->d_flags, h.size() * sizeof(unsigned), cudaMemcpyDeviceToHost, side);
+            cudaStreamSynchronize(side);
+            fprintf(stderr, "[fused HANG] N=%d nspec=%lld grid=%d NT=%d na=%d GS=%d RING=%d ngroups=%d TPG=%d | rankA=%u rankB=%u arrived=%u\n",
+                    s->N, nspec, s->fgrid, NT, s->fna, s->fGS, s->fRING, ngroups, s->N2 / 16, h[0], h[1], h[2]);
+            int mx = 0, mn = 1 << 30, nz = 0;
+            for (int i = 0; i < 512; i++) { const int v = (int)h[4 + i]; if (v) { nz++; if (v > mx) mx = v; if (v < mn) mn = v; } }
+            fprintf(stderr, "  SMs seen %d, CTAs per SM min %d max %d\n", nz, mn, mx);
+            for (int g = 0; g < ngroups && g < 40; g++)
+                fprintf(stderr, "  g=%d a_done=%u b_done=%u\n", g, h[FUSED_ROLE_WORDS + g], h[FUSED_ROLE_WORDS + s->fcap + g]);
+            abort();
+        }
     }
     return 0;
 }
@@ -609,17 +612,24 @@ static int create_impl(spec_ctx* s) {
         size_t zb = (zmb << 20) / ((size_t)N * sizeof(float4));
         s->zbatch = (int)(zb < 1 ? 1 : zb);
         if (s->fused) {
-            // ring = two rounds of B jobs (every CTA holds one job of 16*NT points) plus two groups
             InputView none{nullptr, nullptr, 0};
             int rc = fused_dispatch(s, true, none, 0, 0, nullptr);
             if (rc) return rc;
             const int NT = (s->N2 == 4096) ? 256 : 128;
             s->fGS = (s->N2 >= 512) ? 16 : 64;
+            if (N == 65536) s->fGS = 8;
             if (const char* e = getenv("SPEC_FUSED_GS")) { const int v = atoi(e); if (v >= 2 && v <= 4096 && !(v & (v - 1))) s->fGS = v; }
-            if (const char* e = getenv("SPEC_FUSED_DEPTH")) { const int v = atoi(e); if (v >= 1 && v <= 4096) s->fdepth = v; }
-            const long long round_spectra = ((long long)s->fgrid * NT * 16 + N - 1) / N;
-            long long rs = 2 * round_spectra + 2 * s->fGS;
-            s->fRING = (int)((rs + s->fGS - 1) / s->fGS);
+            // producer share of the resident CTAs: the FIR makes an A task about as long as the row FFT of
+            // the same samples; without it (direct-FFT mode) one producer feeds three consumers
+            s->fna = (NT == 256) ? 1 : ((s->mode == SPEC_MODE_PFB) ? 2 : 1);
+            if (const char* e = getenv("SPEC_FUSED_NA")) { const int v = atoi(e); if (v >= 1 && v < 512 / NT) s->fna = v; }
+            // ring = what the producers (one task each) and the consumers (one job of 16*NT points each)
+            // hold at a time, plus two groups of slack
+            const int per_sm = 512 / NT, nsm = s->fgrid / per_sm;
+            const int tpg = s->N2 / 16;
+            const int a_groups = (nsm * s->fna + tpg - 1) / tpg;
+            const long long b_spectra = ((long long)nsm * (per_sm - s->fna) * NT * 16 + N - 1) / N;
+            s->fRING = a_groups + (int)((b_spectra + s->fGS - 1) / s->fGS) + 2;
             if (const char* e = getenv("SPEC_FUSED_RING")) { const int v = atoi(e); if (v >= 2 && v <= 4096) s->fRING = v; }
             s->zbatch = s->fRING * s->fGS;
         }
