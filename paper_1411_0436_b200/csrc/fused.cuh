@@ -27,6 +27,8 @@
 
 namespace spk {
 
+constexpr int kFusedRoleWords = 516;   // 4 counters + 512 per-SM arrival counters (keeps what follows 16-byte aligned)
+
 struct FusedParams {
     InputView view;        // history ++ input; spectrum j of this launch uses blocks j .. j+T-1
     const float* h;        // T*N coefficients (PFB)
@@ -43,7 +45,9 @@ struct FusedParams {
     int RING;              // groups in the Z ring
     int lgTPG;             // log2 of the A tasks (column tiles of 16) per group, TPG = N2 / 16
     int na_per_sm;         // producer CTAs per SM (the others consume)
-    unsigned* role;        // [0] producer rank counter, [1] consumer rank counter, [2] arrivals, [4 + smid] CTAs seen on that SM
+    unsigned* role;        // [0] producer rank counter, [1] consumer rank counter, [2] arrivals, [3] departures,
+                           // [4 + smid] CTAs seen on that SM.  All counters are zero between launches: the last
+                           // CTA to leave resets them, so a call needs no memset
     unsigned* a_done;      // [group] finished A tasks          } zeroed before every launch; one counter per
     unsigned* b_done;      // [group] consumed rows (of GS*16)  } GROUP of the launch: no epochs, no divisions
     unsigned long long* dbg;  // optional per-CTA counters (SPEC_FUSED_DEBUG): 8 words per CTA
@@ -233,9 +237,21 @@ k_fused(const FusedParams p) {
     __syncthreads();
     // No CTA may leave before every CTA of the grid has arrived: an early exit would free a slot on its
     // SM, a late CTA would land there as a fifth arrival and the per-SM role split would be off.
-    auto leave = [&]() {
-        if (tid == 0)
+    const uint32_t tmem_base_ = tmem_base;
+    auto finish = [&]() {
+        __syncthreads();
+        if (tid == 0) {
             while (ld_relaxed_u32(p.role + 2) < gridDim.x) __nanosleep(200);
+            __threadfence();
+            s_role[0] = (atomicAdd(p.role + 3, 1u) == gridDim.x - 1);   // am I the last one out?
+        }
+        __syncthreads();
+        if (s_role[0]) {
+            __threadfence();
+            for (int i = tid; i < ngroups; i += NT) { p.a_done[i] = 0u; p.b_done[i] = 0u; }
+            for (int i = tid; i < kFusedRoleWords; i += NT) p.role[i] = 0u;
+        }
+        tmem_free_cta<TCOLS>(tmem_base_);
     };
     const bool is_a = s_role[0] != 0;
     const int rank = s_role[1];
@@ -261,8 +277,7 @@ k_fused(const FusedParams p) {
             });   // ends with a __syncthreads
             if (tid == 0) red_release_u32(p.a_done + g, 1u);   // all Z stores of the CTA are ordered before it
         }
-        leave();
-        tmem_free_cta<TCOLS>(tmem_base);
+        finish();
         return;
     }
 
@@ -382,8 +397,7 @@ k_fused(const FusedParams p) {
         if (zpos >= RS) zpos -= RS;
     }
     if (wcur >= 0) sink.flush(st, row, t, wcur);
-    leave();
-    tmem_free_cta<TCOLS>(tmem_base);
+    finish();
 }
 
 }  // namespace spk

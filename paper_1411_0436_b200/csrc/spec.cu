@@ -197,19 +197,21 @@ static void default_coeffs(const spec_ctx* s, std::vector<float>& h) {
 
 // ------------------------------------------------------------------ small kernels
 // read-out: position order [pos][S] -> planar natural order [S][N]  (PAPER.md:95 step 6)
-__global__ void k_unpermute(const float* __restrict__ acc, const int* __restrict__ perm, float* __restrict__ out,
+__global__ void k_unpermute(float* __restrict__ acc, const int* __restrict__ perm, float* __restrict__ out,
                             int N, int S) {
     const int a = blockIdx.x * blockDim.x + threadIdx.x;
     if (a >= N) return;
     const int k = perm[a];
     if (S == 4) {
         const float4 v = ((const float4*)acc)[a];
+        ((float4*)acc)[a] = make_float4(0.f, 0.f, 0.f, 0.f);   // read and clear: a free ring slot is always zero
         out[k] = v.x;
         out[(size_t)N + k] = v.y;
         out[(size_t)2 * N + k] = v.z;
         out[(size_t)3 * N + k] = v.w;
     } else {
         out[k] = acc[a];
+        acc[a] = 0.f;
     }
 }
 
@@ -454,7 +456,7 @@ static int run_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
 }
 
 // ---- fused persistent four-step kernel (fused.cuh): one launch per call
-static const int FUSED_ROLE_WORDS = 516;   // 2 rank counters (+2 pad), 512 per-SM arrival counters; keeps the rest 16-byte aligned
+static const int FUSED_ROLE_WORDS = kFusedRoleWords;
 template <class PL, int NT, int MODE_PFB>
 static int fused_do(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
     auto kern = k_fused<PL, NT, MODE_PFB>;
@@ -480,6 +482,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         s->fcap = 0;
         const int cap = (ngroups + ngroups / 2 + 64) & ~3;   // counters are prefetched as 16-byte lines
         CK(cudaMalloc(&s->d_flags, (size_t)(FUSED_ROLE_WORDS + 2 * cap) * sizeof(unsigned)));
+        CK(cudaMemset(s->d_flags, 0, (size_t)(FUSED_ROLE_WORDS + 2 * cap) * sizeof(unsigned)));   // the kernel leaves them zero
         s->fcap = cap;
     }
     FusedParams p;
@@ -489,7 +492,6 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / 16); p.na_per_sm = s->fna;
     p.role = s->d_flags; p.a_done = s->d_flags + FUSED_ROLE_WORDS; p.b_done = s->d_flags + FUSED_ROLE_WORDS + s->fcap;
     p.dbg = nullptr;
-    CK(cudaMemsetAsync(s->d_flags, 0, (size_t)(FUSED_ROLE_WORDS + 2 * s->fcap) * sizeof(unsigned), st));
     {
         ProfScope ps(s, 0, st);
         kern<<<dim3(s->fgrid), NT, smem, st>>>(p);
@@ -570,6 +572,7 @@ static void free_all(spec_ctx* s) {
 static int alloc_ring(spec_ctx* s, int nslots) {
     float* r = nullptr;
     CK(cudaMalloc(&r, (size_t)(nslots + 1) * acc_floats(s) * sizeof(float)));
+    CK(cudaMemset(r, 0, (size_t)(nslots + 1) * acc_floats(s) * sizeof(float)));   // slots stay zero while free (k_unpermute clears)
     cudaFree(s->d_ring);
     s->d_ring = r;
     s->nring = nslots + 1;
@@ -704,6 +707,7 @@ extern "C" int spec_reset(spec_t* s) {
     if (!s) return SPEC_ERR_ARG;
     CK(cudaDeviceSynchronize());
     s->nhist = 0; s->cur = 0; s->count = 0; s->win_read = 0;
+    CK(cudaMemset(s->d_ring, 0, (size_t)s->nring * acc_floats(s) * sizeof(float)));
     return SPEC_OK;
 }
 
@@ -731,17 +735,6 @@ extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* 
     InputView view{s->d_hist[s->cur], (const uint8_t*)d_in, s->nhist};
     const long long c = s->count + nspec;
     if (nspec > 0) {
-        // zero the ring slots of every window that starts inside this call (at most two memsets)
-        const long long wfirst = (s->count + s->M - 1) / s->M;  // first window starting at or after count
-        const long long wlast = (c - 1) / s->M;                  // last window touched
-        if (wlast >= wfirst) {
-            const long long nw = wlast - wfirst + 1;
-            const long long s0 = wfirst % s->nring;
-            const long long n0 = (s0 + nw <= s->nring) ? nw : s->nring - s0;
-            const size_t ab = acc_floats(s) * sizeof(float);
-            CK(cudaMemsetAsync(s->d_ring + (size_t)s0 * acc_floats(s), 0, (size_t)n0 * ab, st));
-            if (nw > n0) CK(cudaMemsetAsync(s->d_ring, 0, (size_t)(nw - n0) * ab, st));
-        }
         int rc = run_spectra(s, view, 0, nspec, s->count, st);
         if (rc) return rc;
     }
@@ -771,7 +764,7 @@ extern "C" int spec_read_accum(spec_t* s, float* dst, int dst_is_device, void* c
     if (!s || !dst) return SPEC_ERR_ARG;
     if (windows_done(s) - s->win_read <= 0) return 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const float* acc = s->d_ring + (size_t)(s->win_read % s->nring) * acc_floats(s);
+    float* acc = s->d_ring + (size_t)(s->win_read % s->nring) * acc_floats(s);
     float* out = dst_is_device ? dst : s->d_stage;
     {
         ProfScope ps(s, 3, st);
