@@ -286,6 +286,10 @@ def run_ours(a):
     # dominant kernel and its roofline (per-launch averages over the timed region)
     kern = max(("single", "passA", "passB"), key=lambda k: prof[k][0])
     k_ms, k_n = prof[kern]
+    fused = (pfb and 1024 <= N <= 65536) or (not pfb and 8192 <= N <= 65536)
+    kern_name = {"single": "k_fused (persistent four-step: unpack+FIR+FFT+Stokes+accumulate)" if fused
+                 else "k_engine (single-CTA unpack+window+FFT+Stokes+accumulate)",
+                 "passA": "four-step pass A", "passB": "four-step pass B"}[kern]
     flops_total = kernel_flops_per_sample(kern, N, n1, T, pfb) * step_samples * a.steps
     achieved = flops_total / (k_ms * 1e-3) / 1e12 if k_ms > 0 else None
     traffic = None
@@ -317,8 +321,11 @@ def run_ours(a):
                 "h2d_gbs": step_samples * 4 * a.steps / (ms_e2e * 1e-3) / 1e9},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": {"bound": "alu", "kernel": kern, "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
+        "roofline": {"bound": "alu", "kernel": kern, "kernel_name": kern_name, "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
                      "frac": (achieved / fp32_peak) if achieved else None, "traffic": traffic,
+                     "traffic_note": "dram bytes read+write per launch from the ncu --set full capture listed in "
+                                     "profiles/traffic.json (algorithmic: 4 B per dual-pol sample)",
+                     "algorithmic_bytes_per_launch": 4 * step_samples // CALLS_PER_STEP,
                      "peak_source": "spec_measure_fp32_peak in this run (FFMA chains, all SMs); "
                                     "MEASURED_PEAKS.json has no fp32 figure",
                      "peak_nominal": NOMINAL_FP32_TFLOPS, "launches": int(k_n),

@@ -45,6 +45,7 @@ struct FusedParams {
     int RING;              // groups in the Z ring
     int lgTPG;             // log2 of the A tasks (column tiles of 16) per group, TPG = N2 / 16
     int na_per_sm;         // producer CTAs per SM (the others consume)
+    int per_sm;            // resident CTAs per SM (the register budget of the kernel allows exactly this many)
     unsigned* role;        // [0] producer rank counter, [1] consumer rank counter, [2] arrivals, [3] departures,
                            // [4 + smid] CTAs seen on that SM.  All counters are zero between launches: the last
                            // CTA to leave resets them, so a call needs no memset
@@ -198,8 +199,8 @@ __device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, 
 }
 
 // ---------------------------------------------------------------- the kernel
-template <class PL, int NT, int MODE_PFB>
-__global__ void __launch_bounds__(NT, 512 / NT)
+template <class PL, int NT, int MODE_PFB, int PER_SM>
+__global__ void __launch_bounds__(NT, PER_SM)
 k_fused(const FusedParams p) {
     constexpr int L = PL::L, RA = PL::RA, RB = PL::RB, RC = PL::RC, NST = PL::NST;
     constexpr int LA = PL::LA, LB = PL::LB, NTS = PL::NTS;
@@ -255,7 +256,7 @@ k_fused(const FusedParams p) {
     };
     const bool is_a = s_role[0] != 0;
     const int rank = s_role[1];
-    const int per_sm = 512 / NT;
+    const int per_sm = PER_SM;
     const int nsm = (int)gridDim.x / per_sm;
     auto prefetch_line = [&](const unsigned* src) {
         asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(s_pf)), "l"(src) : "memory");
@@ -383,7 +384,10 @@ k_fused(const FusedParams p) {
             }
         }
         if (NST == 3) {
-            __syncthreads();
+            // stage b -> c only exchanges data inside groups of LB = 16 adjacent threads (one block of
+            // LA points), so a warp-level barrier is enough
+            static_assert(NST != 3 || (LB == 16 && RC == 16), "stage c reads what its own half-warp wrote");
+            __syncwarp();
             if (active) {
                 cpx v[RC];
 #pragma unroll

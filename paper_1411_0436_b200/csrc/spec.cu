@@ -457,9 +457,12 @@ static int run_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
 
 // ---- fused persistent four-step kernel (fused.cuh): one launch per call
 static const int FUSED_ROLE_WORDS = kFusedRoleWords;
-template <class PL, int NT, int MODE_PFB>
+#ifndef FUSED_PER_SM
+#define FUSED_PER_SM 4   // resident CTAs of 128 threads per SM (128 registers each)
+#endif
+template <class PL, int NT, int MODE_PFB, int PER_SM>
 static int fused_do(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
-    auto kern = k_fused<PL, NT, MODE_PFB>;
+    auto kern = k_fused<PL, NT, MODE_PFB, PER_SM>;
     const size_t smem = (size_t)NT * 16 * sizeof(float4);
     if (query) {
         int rc = prep_smem(kern, smem);
@@ -468,8 +471,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         // columns and 4 x 33 KB of shared memory fit.  The occupancy API cannot be asked: it reports 1
         // for any kernel that contains tcgen05.alloc (measured: 4 such CTAs of 128 threads do share an
         // SM), which also rules out cudaLaunchCooperativeKernel for a grid of this size.
-        int per_sm = 512 / NT;
-        if (const char* e = getenv("SPEC_FUSED_CTAS")) { const int v = atoi(e); if (v >= 1 && v <= per_sm) per_sm = v; }
+        const int per_sm = PER_SM;
         s->fgrid = per_sm * s->numSM;
         return 0;
     }
@@ -489,7 +491,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     p.view = view; p.h = s->d_coef; p.Z = s->d_Z; p.twN = s->d_twN; p.twL = s->d_tw2;
     p.ring = s->d_ring; p.acc_stride = acc_floats(s); p.nring = s->nring;
     p.N = s->N; p.N2 = s->N2; p.nspec = (int)nspec; p.c0 = c0; p.M = s->M;
-    p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / 16); p.na_per_sm = s->fna;
+    p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / 16); p.na_per_sm = s->fna; p.per_sm = PER_SM;
     p.role = s->d_flags; p.a_done = s->d_flags + FUSED_ROLE_WORDS; p.b_done = s->d_flags + FUSED_ROLE_WORDS + s->fcap;
     p.dbg = nullptr;
     {
@@ -524,18 +526,18 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
 static int fused_dispatch(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
     const bool pfb = (s->mode == SPEC_MODE_PFB);
     switch (s->N2) {
-#define F_CASE(LEN, PLX, NT)                                                         \
+#define F_CASE(LEN, PLX, NT, PS)                                                     \
     case LEN:                                                                        \
-        return pfb ? fused_do<PLX, NT, 1>(s, query, view, nspec, c0, st)             \
-                   : fused_do<PLX, NT, 0>(s, query, view, nspec, c0, st);
-        F_CASE(512, PL512, 128)
-        F_CASE(1024, PL1024, 128)
-        F_CASE(2048, PL2048, 128)
-        F_CASE(4096, PL4096, 256)
+        return pfb ? fused_do<PLX, NT, 1, PS>(s, query, view, nspec, c0, st)         \
+                   : fused_do<PLX, NT, 0, PS>(s, query, view, nspec, c0, st);
+        F_CASE(512, PL512, 128, FUSED_PER_SM)
+        F_CASE(1024, PL1024, 128, FUSED_PER_SM)
+        F_CASE(2048, PL2048, 128, FUSED_PER_SM)
+        F_CASE(4096, PL4096, 256, 2)
 #undef F_CASE
-        case 64: return fused_do<PL64, 128, 1>(s, query, view, nspec, c0, st);
-        case 128: return fused_do<PL128, 128, 1>(s, query, view, nspec, c0, st);
-        case 256: return fused_do<PL256, 128, 1>(s, query, view, nspec, c0, st);
+        case 64: return fused_do<PL64, 128, 1, FUSED_PER_SM>(s, query, view, nspec, c0, st);
+        case 128: return fused_do<PL128, 128, 1, FUSED_PER_SM>(s, query, view, nspec, c0, st);
+        case 256: return fused_do<PL256, 128, 1, FUSED_PER_SM>(s, query, view, nspec, c0, st);
     }
     return SPEC_ERR_ARG;
 }
@@ -625,10 +627,10 @@ static int create_impl(spec_ctx* s) {
             // producer share of the resident CTAs: the FIR makes an A task about as long as the row FFT of
             // the same samples; without it (direct-FFT mode) one producer feeds three consumers
             s->fna = (NT == 256) ? 1 : ((s->mode == SPEC_MODE_PFB) ? 2 : 1);
-            if (const char* e = getenv("SPEC_FUSED_NA")) { const int v = atoi(e); if (v >= 1 && v < 512 / NT) s->fna = v; }
+            if (const char* e = getenv("SPEC_FUSED_NA")) { const int v = atoi(e); if (v >= 1 && v < ((NT == 256) ? 2 : FUSED_PER_SM)) s->fna = v; }
             // ring = what the producers (one task each) and the consumers (one job of 16*NT points each)
             // hold at a time, plus two groups of slack
-            const int per_sm = 512 / NT, nsm = s->fgrid / per_sm;
+            const int per_sm = (NT == 256) ? 2 : FUSED_PER_SM, nsm = s->fgrid / per_sm;
             const int tpg = s->N2 / 16;
             const int a_groups = (nsm * s->fna + tpg - 1) / tpg;
             const long long b_spectra = ((long long)nsm * (per_sm - s->fna) * NT * 16 + N - 1) / N;
