@@ -77,116 +77,108 @@ __device__ __forceinline__ void red_release_u32(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 
-// ---------------------------------------------------------------- A task
+// ---------------------------------------------------------------- A task, PFB mode
 // C = 16 adjacent columns n2 (all 16 rows n1: 256 filter branches), the GS spectra of one group,
-// R = NT/16 spectra per phase.  FIR phase: each thread owns 256/NT branches and slides an 8-sample
-// register window over R+7 blocks (every raw sample of the phase is unpacked once); FFT phase: each
-// thread owns one (spectrum, column) pair.  N is a compile-time constant, so every load and store of
-// a phase is one base register plus an immediate offset.
-template <int NT, int N2, bool RAGGED>
-__device__ __forceinline__ void fused_fir_phase(const FusedParams& p, float4* ysm, const float (&hc)[256 / NT][8],
-                                                const int (&nbr)[256 / NT], int mg, int j0, int nsp) {
-    constexpr int C = 16, R = NT / C, T = 8, N = 16 * N2, BPT = 256 / NT;
-    const int tid = threadIdx.x;
-    const int qmax = nsp - 1 - j0 + (T - 1);  // last valid block of this phase (ragged tail only)
-    uint32_t raw[BPT][R + T - 1];
-    const bool in_input = (mg + j0 >= p.view.nhist);
+// R = NT/16 spectra per phase.  The raw samples of a phase (R+7 blocks x 16 rows x 64 bytes) are
+// staged in shared memory with 16-byte cp.async copies issued ONE PHASE AHEAD (across task
+// boundaries too: the task list of a producer is static), so the latency of the input stream is
+// hidden behind the previous phase's column FFTs.  FIR phase: each thread owns 256/NT branches and
+// slides an 8-sample register window over the R+7 blocks (every raw sample is unpacked once per
+// phase); FFT phase: each thread owns one (spectrum, column) pair.
+template <int NT, int N2>
+struct ProducerPfb {
+    static constexpr int C = 16, R = NT / C, T = 8, N = 16 * N2, BPT = 256 / NT;
+    static constexpr int NBLK = R + T - 1;                 // blocks per phase
+    static constexpr int RAW_WORDS = NBLK * 256;           // u32 per staged tile
+    static constexpr int CHUNKS = RAW_WORDS / 4;           // 16-byte copies per tile
+
+    // issue the copies of phase (g, tile, j0): block q of the phase is view block mg + j0 + min(q, qmax)
+    static __device__ __forceinline__ void stage(const FusedParams& p, uint32_t* rawsm, int g, int tile, int j0) {
+        const int GS = 1 << p.lgGS;
+        const int mg = g << p.lgGS;
+        const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;
+        const int qmax = nsp - 1 - j0 + (T - 1);
+        const int n2_0 = tile * C;
 #pragma unroll
-    for (int i = 0; i < BPT; i++) {
-        if (in_input) {
-            const uint32_t* base = (const uint32_t*)p.view.in + (size_t)(mg + j0 - p.view.nhist) * N + nbr[i];
-#pragma unroll
-            for (int q = 0; q < R + T - 1; q++)
-                raw[i][q] = RAGGED ? __ldg(base + (size_t)(q < qmax ? q : qmax) * N) : __ldg(base + q * N);
-        } else {
-#pragma unroll
-            for (int q = 0; q < R + T - 1; q++)
-                raw[i][q] = fetch_raw<2>(p.view, mg + j0 + ((!RAGGED || q < qmax) ? q : qmax), nbr[i], N);
-        }
-    }
-#pragma unroll
-    for (int i = 0; i < BPT; i++) {
-        const int beta = tid + NT * i;
-        const int n1 = beta / C, c = beta % C;
-        cpx x[T];
-#pragma unroll
-        for (int t = 0; t < T - 1; t++) x[t] = unpack_cpx<2>(raw[i][t]);
-#pragma unroll
-        for (int r = 0; r < R; r++) {
-            x[(r + T - 1) % T] = unpack_cpx<2>(raw[i][r + T - 1]);
-            u64 re = 0ull, im = 0ull;
-#pragma unroll
-            for (int t = 0; t < T; t++) {
-                re = fma2(x[(r + t) % T].re, bc(hc[i][t]), re);
-                im = fma2(x[(r + t) % T].im, bc(hc[i][t]), im);
+        for (int i = 0; i < (CHUNKS + NT - 1) / NT; i++) {
+            const int c = threadIdx.x + NT * i;
+            if (CHUNKS % NT == 0 || c < CHUNKS) {
+                const int q = c >> 6, n1 = (c >> 2) & 15, part = c & 3;
+                const int blk = mg + j0 + (q < qmax ? q : qmax);
+                const uint8_t* base = (blk < p.view.nhist) ? p.view.hist + (size_t)blk * N * 4
+                                                           : p.view.in + (size_t)(blk - p.view.nhist) * N * 4;
+                const uint8_t* src = base + ((size_t)n1 * N2 + n2_0) * 4 + part * 16;
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(rawsm + c * 4)), "l"(src) : "memory");
             }
-            ysm[(r * 16 + n1) * C + c] = cpx_to_f4({re, im});
         }
     }
-}
+};
 
-// `wait_room` (called by thread 0 only) returns once the ring slot of group g may be overwritten; it
-// sits in front of the first barrier that precedes a Z store, so the loads and the FIR of the first
-// phase overlap the wait.
-template <int NT, int MODE_PFB, int N2, class WaitRoom>
-__device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, int g, int tile, WaitRoom wait_room) {
-    constexpr int C = 16, R = NT / C, T = 8, N = 16 * N2;
-    constexpr int BPT = 256 / NT;  // branches per thread in the FIR phase
+// The producer loop of one CTA in PFB mode: tasks rank, rank + NA, ...; `wait_room(g)` (thread 0) returns
+// once the ring slot of group g may be overwritten, `signal(g, next task)` (thread 0) publishes a finished task.
+template <int NT, int N2, class WaitRoom, class Signal>
+__device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4* smem, int rank, int NA, int natasks,
+                                                   WaitRoom wait_room, Signal signal) {
+    typedef ProducerPfb<NT, N2> PP;
+    constexpr int C = PP::C, R = PP::R, T = PP::T, N = PP::N, BPT = PP::BPT;
+    float4* const ysm = smem;                                   // [R][16][C] FIR outputs
+    uint32_t* const rawsm = (uint32_t*)(smem + R * 16 * C);     // [R+7][16][C] raw samples of the phase
     const int tid = threadIdx.x;
-    const int n2_0 = tile * C;
     const int GS = 1 << p.lgGS;
-    const int mg = g << p.lgGS;                                   // first spectrum of the group
-    const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;      // valid spectra in it
+    const int TPGm = (1 << p.lgTPG) - 1;
     const int fr = tid / C, fc = tid % C;
-    const int n2 = n2_0 + fc;
-    float4* const zg = p.Z + ((size_t)((unsigned)g % (unsigned)p.RING) << p.lgGS) * N + n2;
 
-    float2 tw[16];
+    if (rank < natasks) PP::stage(p, rawsm, rank >> p.lgTPG, rank & TPGm, 0);
+    for (int a = rank; a < natasks; a += NA) {
+        const int g = a >> p.lgTPG, tile = a & TPGm;
+        const int n2_0 = tile * C;
+        const int mg = g << p.lgGS;
+        const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;
+        const int n2 = n2_0 + fc;
+        float4* const zg = p.Z + ((size_t)((unsigned)g % (unsigned)p.RING) << p.lgGS) * N + n2;
+        float2 tw[16];
 #pragma unroll
-    for (int k = 1; k < 16; k++) tw[k] = __ldg(p.twN + (size_t)n2 * k);
-
-    if (MODE_PFB) {
+        for (int k = 1; k < 16; k++) tw[k] = __ldg(p.twN + (size_t)n2 * k);
         float hc[BPT][T];
-        int nbr[BPT];
 #pragma unroll
         for (int i = 0; i < BPT; i++) {
             const int beta = tid + NT * i;
-            nbr[i] = (beta / C) * N2 + n2_0 + (beta % C);
+            const int nbr = (beta / C) * N2 + n2_0 + (beta % C);
 #pragma unroll
-            for (int t = 0; t < T; t++) hc[i][t] = __ldg(p.h + t * N + nbr[i]);
+            for (int t = 0; t < T; t++) hc[i][t] = __ldg(p.h + t * N + nbr);
         }
         for (int j0 = 0; j0 < nsp; j0 += R) {
-            if (j0 + R <= nsp) fused_fir_phase<NT, N2, false>(p, ysm, hc, nbr, mg, j0, nsp);
-            else fused_fir_phase<NT, N2, true>(p, ysm, hc, nbr, mg, j0, nsp);
-            if (j0 == 0 && tid == 0) wait_room();
-            __syncthreads();
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            __syncthreads();   // the staged tile is complete; the previous phase's column FFTs have read ysm
+            // ---------------- FIR phase
+#pragma unroll
+            for (int i = 0; i < BPT; i++) {
+                const int beta = tid + NT * i;
+                cpx x[T];
+#pragma unroll
+                for (int t = 0; t < T - 1; t++) x[t] = unpack_cpx<2>(rawsm[t * 256 + beta]);
+#pragma unroll
+                for (int r = 0; r < R; r++) {
+                    x[(r + T - 1) % T] = unpack_cpx<2>(rawsm[(r + T - 1) * 256 + beta]);
+                    u64 re = 0ull, im = 0ull;
+#pragma unroll
+                    for (int t = 0; t < T; t++) {
+                        re = fma2(x[(r + t) % T].re, bc(hc[i][t]), re);
+                        im = fma2(x[(r + t) % T].im, bc(hc[i][t]), im);
+                    }
+                    ysm[r * 256 + beta] = cpx_to_f4({re, im});
+                }
+            }
+            if (j0 == 0 && tid == 0) wait_room(g);
+            __syncthreads();   // ysm complete, the raw tile is free again
+            // ---------------- stage the next phase (of this task or of my next task)
+            if (j0 + R < nsp) PP::stage(p, rawsm, g, tile, j0 + R);
+            else if (a + NA < natasks) PP::stage(p, rawsm, (a + NA) >> p.lgTPG, (a + NA) & TPGm, 0);
             // ---------------- column FFT phase
             if (j0 + fr < nsp) {
                 cpx v[16];
 #pragma unroll
-                for (int n1 = 0; n1 < 16; n1++) v[n1] = f4_to_cpx(ysm[(fr * 16 + n1) * C + fc]);
-                dft<16>(v);
-                float4* zp = zg + (size_t)(j0 + fr) * N;
-                zp[0] = cpx_to_f4(v[0]);
-#pragma unroll
-                for (int k = 1; k < 16; k++) zp[k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
-            }
-            __syncthreads();
-        }
-    } else {
-        // direct-FFT mode: no pre-filter, the 16 samples of a column go straight from
-        // global memory through the unpack into the butterfly
-        if (tid == 0) wait_room();
-        __syncthreads();
-        for (int j0 = 0; j0 < nsp; j0 += R) {
-            if (j0 + fr < nsp) {
-                const uint32_t* base = (const uint32_t*)p.view.in + (size_t)(mg + j0 + fr) * N + n2;
-                uint32_t raw[16];
-#pragma unroll
-                for (int n1 = 0; n1 < 16; n1++) raw[n1] = __ldg(base + n1 * N2);
-                cpx v[16];
-#pragma unroll
-                for (int n1 = 0; n1 < 16; n1++) v[n1] = unpack_cpx<2>(raw[n1]);
+                for (int n1 = 0; n1 < 16; n1++) v[n1] = f4_to_cpx(ysm[fr * 256 + n1 * C + fc]);
                 dft<16>(v);
                 float4* zp = zg + (size_t)(j0 + fr) * N;
                 zp[0] = cpx_to_f4(v[0]);
@@ -194,8 +186,45 @@ __device__ __forceinline__ void fused_task_A(const FusedParams& p, float4* ysm, 
                 for (int k = 1; k < 16; k++) zp[k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
             }
         }
-        __syncthreads();
+        __syncthreads();   // every Z store of the task has been issued by its thread
+        if (tid == 0) signal(g, a + NA);
     }
+}
+
+// One A task in direct-FFT mode: no pre-filter, the 16 samples of a column go straight
+// from global memory through the unpack into the butterfly.
+template <int NT, int N2, class WaitRoom>
+__device__ __forceinline__ void fused_task_A_fft(const FusedParams& p, int g, int tile, WaitRoom wait_room) {
+    constexpr int C = 16, R = NT / C, N = 16 * N2;
+    const int tid = threadIdx.x;
+    const int GS = 1 << p.lgGS;
+    const int mg = g << p.lgGS;
+    const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;
+    const int fr = tid / C, fc = tid % C;
+    const int n2 = tile * C + fc;
+    float4* const zg = p.Z + ((size_t)((unsigned)g % (unsigned)p.RING) << p.lgGS) * N + n2;
+    float2 tw[16];
+#pragma unroll
+    for (int k = 1; k < 16; k++) tw[k] = __ldg(p.twN + (size_t)n2 * k);
+    if (tid == 0) wait_room(g);
+    __syncthreads();
+    for (int j0 = 0; j0 < nsp; j0 += R) {
+        if (j0 + fr < nsp) {
+            const uint32_t* base = (const uint32_t*)p.view.in + (size_t)(mg + j0 + fr) * N + n2;
+            uint32_t raw[16];
+#pragma unroll
+            for (int n1 = 0; n1 < 16; n1++) raw[n1] = __ldg(base + n1 * N2);
+            cpx v[16];
+#pragma unroll
+            for (int n1 = 0; n1 < 16; n1++) v[n1] = unpack_cpx<2>(raw[n1]);
+            dft<16>(v);
+            float4* zp = zg + (size_t)(j0 + fr) * N;
+            zp[0] = cpx_to_f4(v[0]);
+#pragma unroll
+            for (int k = 1; k < 16; k++) zp[k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
+        }
+    }
+    __syncthreads();
 }
 
 // ---------------------------------------------------------------- the kernel
@@ -209,7 +238,7 @@ k_fused(const FusedParams p) {
     constexpr int SPJ = (G >= 16) ? G / 16 : 1;     // spectra per B job
     constexpr int TCOLS = (NT > 128) ? 128 : 64;
     static_assert(NST >= 2 && PL::RLAST == 16 && G * L * 16 == NT * 256, "row plan");
-    extern __shared__ float4 smem[];                // G*L float4: B exchange buffer / A FIR hand-off
+    extern __shared__ float4 smem[];                // G*L float4: B exchange buffer / A FIR hand-off (+ the staged raw tile)
     __shared__ int s_role[2];
     __shared__ uint32_t s_tmem;
     __shared__ __align__(16) unsigned s_pf[4];      // landing zone of the prefetched counter line
@@ -266,17 +295,36 @@ k_fused(const FusedParams p) {
         // ================= producer: A tasks rank, rank + NA, ...
         const int NA = nsm * p.na_per_sm;
         const int natasks = ngroups << p.lgTPG;
-        for (int a = rank; a < natasks; a += NA) {
-            const int g = a >> p.lgTPG;
+        int pf_g = -1;   // thread 0: group whose b_done line was prefetched into s_pf
+        auto wait_room = [&](int g) {
             const int gfree = g - p.RING;     // the group whose ring slot this task overwrites
-            if (tid == 0 && gfree >= 0) prefetch_line(p.b_done + (gfree & ~3));
-            fused_task_A<NT, MODE_PFB, L>(p, smem, g, a & (int)(TPG - 1), [&]() {
-                if (gfree < 0) return;
+            if (gfree < 0) return;
+            if (pf_g == gfree) {
                 asm volatile("cp.async.wait_all;" ::: "memory");
                 if (*(volatile unsigned*)&s_pf[gfree & 3] >= rows_full) return;
-                while (ld_relaxed_u32(p.b_done + gfree) < rows_full) __nanosleep(200);
-            });   // ends with a __syncthreads
-            if (tid == 0) red_release_u32(p.a_done + g, 1u);   // all Z stores of the CTA are ordered before it
+            }
+            while (ld_relaxed_u32(p.b_done + gfree) < rows_full) __nanosleep(200);
+        };
+        auto prefetch_room = [&](int a) {    // thread 0, for my task a (if any)
+            pf_g = -1;
+            if (a < natasks && (a >> p.lgTPG) >= p.RING) {
+                pf_g = (a >> p.lgTPG) - p.RING;
+                prefetch_line(p.b_done + (pf_g & ~3));
+            }
+        };
+        if (MODE_PFB) {
+            if (tid == 0) prefetch_room(rank);
+            fused_producer_pfb<NT, L>(p, smem, rank, NA, natasks, wait_room, [&](int g, int a_next) {
+                red_release_u32(p.a_done + g, 1u);   // all Z stores of the CTA are ordered before it
+                prefetch_room(a_next);
+            });
+        } else {
+            for (int a = rank; a < natasks; a += NA) {
+                const int g = a >> p.lgTPG;
+                if (tid == 0) prefetch_room(a);
+                fused_task_A_fft<NT, L>(p, g, a & (int)(TPG - 1), wait_room);   // ends with a __syncthreads
+                if (tid == 0) red_release_u32(p.a_done + g, 1u);
+            }
         }
         finish();
         return;

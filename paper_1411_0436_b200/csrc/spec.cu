@@ -463,7 +463,8 @@ static const int FUSED_ROLE_WORDS = kFusedRoleWords;
 template <class PL, int NT, int MODE_PFB, int PER_SM>
 static int fused_do(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
     auto kern = k_fused<PL, NT, MODE_PFB, PER_SM>;
-    const size_t smem = (size_t)NT * 16 * sizeof(float4);
+    // exchange buffer / FIR hand-off, plus (PFB) the staged raw tile of a producer phase: R+7 blocks of 1 KiB
+    const size_t smem = (size_t)NT * 16 * sizeof(float4) + (MODE_PFB ? (size_t)(NT / 16 + 7) * 1024 : 0);
     if (query) {
         int rc = prep_smem(kern, smem);
         if (rc) return rc;
