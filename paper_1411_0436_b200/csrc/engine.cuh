@@ -259,9 +259,11 @@ struct SinkStokesTmem {
     struct State {
         uint32_t taddr;
     };
-    __device__ __forceinline__ void init(State& s, uint32_t tmem_base) const {
+    // colstride: columns reserved per set of four warps (64 accumulator words, plus whatever else the
+    // kernel keeps in the thread's lane)
+    __device__ __forceinline__ void init(State& s, uint32_t tmem_base, int colstride = 64) const {
         const int warp = threadIdx.x >> 5;
-        s.taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)(warp >> 2) * 64;
+        s.taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * colstride);
     }
     __device__ __forceinline__ void begin(State& s) const {
         float z[32];

@@ -51,7 +51,7 @@ struct FusedParams {
                            // CTA to leave resets them, so a call needs no memset
     unsigned* a_done;      // [group] finished A tasks          } zeroed before every launch; one counter per
     unsigned* b_done;      // [group] consumed rows (of GS*16)  } GROUP of the launch: no epochs, no divisions
-    unsigned long long* dbg;  // optional per-CTA counters (SPEC_FUSED_DEBUG): 8 words per CTA
+    int dbg_mode;          // timing experiments only (SPEC_FUSED_SKIP): 1 = consumers skip their FFT, 2 = producers skip their work
 };
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
@@ -133,7 +133,7 @@ __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4*
         const int g = a >> p.lgTPG, tile = a & TPGm;
         const int n2_0 = tile * C;
         const int mg = g << p.lgGS;
-        const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;
+        const int nsp = (p.dbg_mode == 2) ? 0 : ((p.nspec - mg < GS) ? p.nspec - mg : GS);
         const int n2 = n2_0 + fc;
         float4* const zg = p.Z + ((size_t)((unsigned)g % (unsigned)p.RING) << p.lgGS) * N + n2;
         float2 tw[16];
@@ -236,7 +236,7 @@ k_fused(const FusedParams p) {
     constexpr int G = NT / NTS;                     // rows per B job
     constexpr int RGN = (G >= 16) ? 1 : 16 / G;     // row groups per spectrum
     constexpr int SPJ = (G >= 16) ? G / 16 : 1;     // spectra per B job
-    constexpr int TCOLS = (NT > 128) ? 128 : 64;
+    constexpr int TCOLS = (NT > 128) ? 256 : 128;   // per set of four warps: 64 accumulator + 64 twiddle columns
     static_assert(NST >= 2 && PL::RLAST == 16 && G * L * 16 == NT * 256, "row plan");
     extern __shared__ float4 smem[];                // G*L float4: B exchange buffer / A FIR hand-off (+ the staged raw tile)
     __shared__ int s_role[2];
@@ -354,8 +354,45 @@ k_fused(const FusedParams p) {
 
     SinkStokesTmem sink{p.ring, p.acc_stride, p.nring, L, 1};
     SinkStokesTmem::State st;
-    sink.init(st, tmem_base);
+    sink.init(st, tmem_base, 128);
     sink.begin(st);
+    // The stage twiddles a thread needs are the same for every job (they depend on its index only):
+    // they are parked in tensor memory next to the accumulators (columns 64.. of the thread's lane) and
+    // fetched with one tcgen05.ld per stage, instead of 29 global loads per job that mostly missed the
+    // small L1 left beside the shared-memory carve-out (measured: 14 of 40 B/sample of L2->SM traffic).
+    constexpr int TWA = (16 / RA) * (RA - 1);                       // float2 per thread, stage a
+    constexpr int TWB = (NST == 3) ? (16 / RB) * (RB - 1) : 0;      // stage b
+    static_assert(TWA <= 16 && TWB <= 16, "32 words per stage");
+    const uint32_t ttw = st.taddr + 64;
+    {
+        float w[32];
+#pragma unroll
+        for (int i = 0; i < 32; i++) w[i] = 0.f;
+#pragma unroll
+        for (int u = 0; u < 16 / RA; u++)
+#pragma unroll
+            for (int q = 1; q < RA; q++) {
+                const float2 x = __ldg(p.twL + (q - 1) * LA + t + NTS * u);
+                w[2 * (u * (RA - 1) + q - 1)] = x.x;
+                w[2 * (u * (RA - 1) + q - 1) + 1] = x.y;
+            }
+        tmem_st32(ttw, w);
+        if (NST == 3) {
+            float w2[32];
+#pragma unroll
+            for (int i = 0; i < 32; i++) w2[i] = 0.f;
+#pragma unroll
+            for (int u = 0; u < 16 / RB; u++)
+#pragma unroll
+                for (int q = 1; q < RB; q++) {
+                    const float2 x = __ldg(p.twL + (RA - 1) * LA + (q - 1) * LB + (t + NTS * u) % LB);
+                    w2[2 * (u * (RB - 1) + q - 1)] = x.x;
+                    w2[2 * (u * (RB - 1) + q - 1) + 1] = x.y;
+                }
+            tmem_st32(ttw + 32, w2);
+        }
+        tmem_wait_st();
+    }
     long long wcur = -1;       // accumulation window the TMEM sums belong to (-1: none yet)
     long long nextb = 0;       // first spectrum (of this launch) that no longer belongs to window wcur
     int ready_g = -1;          // thread 0: newest group known to be complete
@@ -377,7 +414,7 @@ k_fused(const FusedParams p) {
         }
         __syncthreads();   // publishes "group complete"; also frees the exchange buffer of the previous job
         // ---------------- B job bi: spectrum m (ring position zpos), row `row`
-        const bool active = m < p.nspec;
+        const bool active = m < p.nspec && p.dbg_mode != 1;
         if (active && m >= nextb) {   // new accumulation window (warp-uniform: a warp never straddles spectra)
             if (wcur >= 0) { sink.flush(st, row, t, wcur); sink.begin(st); }
             wcur = (p.c0 + m) / p.M;
@@ -386,19 +423,23 @@ k_fused(const FusedParams p) {
         const float4* zrow = p.Z + (size_t)zpos * (16 * L) + row * L;
         // stage a: rows of Z straight from L2 (ld.global.cg: the ring is rewritten by other SMs)
         if (active) {
+            float twa[32];
+            tmem_ld32(ttw, twa);
+            cpx v[16 / RA][RA];
+#pragma unroll
+            for (int u = 0; u < 16 / RA; u++)
+#pragma unroll
+                for (int r = 0; r < RA; r++) v[u][r] = f4_to_cpx(__ldcg(zrow + t + NTS * u + r * LA));
+            tmem_wait_ld();
 #pragma unroll
             for (int u = 0; u < 16 / RA; u++) {
                 const int ja = t + NTS * u;
-                cpx v[RA];
+                dft<RA>(v[u]);
+                smem[addr(ja)] = cpx_to_f4(v[u][0]);
 #pragma unroll
-                for (int r = 0; r < RA; r++) v[r] = f4_to_cpx(__ldcg(zrow + ja + r * LA));
-                dft<RA>(v);
-                smem[addr(ja)] = cpx_to_f4(v[0]);
-#pragma unroll
-                for (int q = 1; q < RA; q++) {
-                    const float2 w = __ldg(p.twL + (q - 1) * LA + ja);
-                    smem[addr(ja + q * LA)] = cpx_to_f4(cmul(v[q], w.x, w.y));
-                }
+                for (int q = 1; q < RA; q++)
+                    smem[addr(ja + q * LA)] = cpx_to_f4(cmul(v[u][q], twa[2 * (u * (RA - 1) + q - 1)],
+                                                             twa[2 * (u * (RA - 1) + q - 1) + 1]));
             }
         }
         __syncthreads();
@@ -410,6 +451,8 @@ k_fused(const FusedParams p) {
             red_release_u32(p.b_done + (s0 >> p.lgGS), (G >= 16) ? (unsigned)(16 * (s1 - s0)) : (unsigned)G);
         }
         if (active) {
+            float twb[32];
+            if (NST == 3) tmem_ld32(ttw + 32, twb);
 #pragma unroll
             for (int u = 0; u < 16 / RB; u++) {
                 const int i = t + NTS * u;
@@ -422,12 +465,12 @@ k_fused(const FusedParams p) {
                 if (NST == 2) {
                     sink.put16(st, m, 0, i, i, RA, v);
                 } else {
+                    if (u == 0) tmem_wait_ld();
                     smem[addr(base)] = cpx_to_f4(v[0]);
 #pragma unroll
-                    for (int q = 1; q < RB; q++) {
-                        const float2 w = __ldg(p.twL + (RA - 1) * LA + (q - 1) * LB + jb);
-                        smem[addr(base + q * LB)] = cpx_to_f4(cmul(v[q], w.x, w.y));
-                    }
+                    for (int q = 1; q < RB; q++)
+                        smem[addr(base + q * LB)] = cpx_to_f4(cmul(v[q], twb[2 * (u * (RB - 1) + q - 1)],
+                                                                  twb[2 * (u * (RB - 1) + q - 1) + 1]));
                 }
             }
         }

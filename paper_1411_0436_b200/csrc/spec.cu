@@ -494,7 +494,8 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     p.N = s->N; p.N2 = s->N2; p.nspec = (int)nspec; p.c0 = c0; p.M = s->M;
     p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / 16); p.na_per_sm = s->fna; p.per_sm = PER_SM;
     p.role = s->d_flags; p.a_done = s->d_flags + FUSED_ROLE_WORDS; p.b_done = s->d_flags + FUSED_ROLE_WORDS + s->fcap;
-    p.dbg = nullptr;
+    p.dbg_mode = 0;
+    if (const char* e = getenv("SPEC_FUSED_SKIP")) p.dbg_mode = atoi(e);
     {
         ProfScope ps(s, 0, st);
         kern<<<dim3(s->fgrid), NT, smem, st>>>(p);
