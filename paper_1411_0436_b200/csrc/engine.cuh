@@ -483,7 +483,10 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                     }
                 }
             }
-            __syncthreads();
+            // three-stage plans: stage c only reads what the same 16 adjacent threads wrote in stage b
+            // (one block of LA points), so a warp-level barrier is enough there
+            if (NST == 3 && !IL && LB == 16 && RC == 16) __syncwarp();
+            else __syncthreads();
         }
         if (NST == 3) {
             // ---------------- stage c
