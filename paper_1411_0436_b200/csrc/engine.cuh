@@ -273,32 +273,53 @@ struct SinkStokesTmem {
         tmem_st32(s.taddr + 32, z);
         tmem_wait_st();
     }
+    static __device__ __forceinline__ void stokes8(float* a, const cpx* v) {
+#pragma unroll
+        for (int j = 0; j < 8; j++) {
+            const cpx x = v[j];
+            u64 pw = pk(a[4 * j], a[4 * j + 1]);
+            pw = fma2(x.re, x.re, pw);
+            pw = fma2(x.im, x.im, pw);
+            upk(pw, a[4 * j], a[4 * j + 1]);
+            float xr, yr, xi, yi;
+            upk(x.re, xr, yr);
+            upk(x.im, xi, yi);
+            a[4 * j + 2] = fmaf(xr, yr, fmaf(xi, yi, a[4 * j + 2]));   // Re(X conj Y) = XrYr + XiYi
+            a[4 * j + 3] = fmaf(xi, yr, fmaf(-xr, yi, a[4 * j + 3]));  // Im(X conj Y) = XiYr - XrYi
+        }
+    }
+    // The stores of one call are only waited for at the start of the next TMEM access of the thread
+    // (next job), so they overlap whatever comes in between.
     __device__ __forceinline__ void put16(State& s, long long, int, int, int, int, const cpx* v) const {
+        tmem_wait_st();
 #pragma unroll
         for (int hh = 0; hh < 2; hh++) {
             float a[32];
             tmem_ld32(s.taddr + 32 * hh, a);
             tmem_wait_ld();
-#pragma unroll
-            for (int j = 0; j < 8; j++) {
-                const cpx x = v[8 * hh + j];
-                u64 pw = pk(a[4 * j], a[4 * j + 1]);
-                pw = fma2(x.re, x.re, pw);
-                pw = fma2(x.im, x.im, pw);
-                upk(pw, a[4 * j], a[4 * j + 1]);
-                float xr, yr, xi, yi;
-                upk(x.re, xr, yr);
-                upk(x.im, xi, yi);
-                a[4 * j + 2] = fmaf(xr, yr, fmaf(xi, yi, a[4 * j + 2]));
-                a[4 * j + 3] = fmaf(xi, yr, fmaf(-xr, yi, a[4 * j + 3]));
-            }
+            stokes8(a, v + 8 * hh);
             tmem_st32(s.taddr + 32 * hh, a);
         }
+    }
+    // split form: `preload` before the last butterfly, `put16_preloaded` after it
+    __device__ __forceinline__ void preload(State& s, float* a0) const {
         tmem_wait_st();
+        tmem_ld32(s.taddr, a0);
+    }
+    __device__ __forceinline__ void put16_preloaded(State& s, float* a0, const cpx* v) const {
+        float a1[32];
+        tmem_wait_ld();
+        tmem_ld32(s.taddr + 32, a1);
+        stokes8(a0, v);
+        tmem_st32(s.taddr, a0);
+        tmem_wait_ld();
+        stokes8(a1, v + 8);
+        tmem_st32(s.taddr + 32, a1);
     }
     __device__ __forceinline__ void flush(State& s, int slot_id, int i, long long w) const {
         float4* acc = (float4*)(ring + (size_t)(w % nring) * stride);
         const size_t pos = (rows_mode ? (size_t)slot_id * slot_len : 0) + (size_t)i * 16;
+        tmem_wait_st();
 #pragma unroll
         for (int hh = 0; hh < 2; hh++) {
             float a[32];

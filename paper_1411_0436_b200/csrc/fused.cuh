@@ -480,11 +480,13 @@ k_fused(const FusedParams p) {
             static_assert(NST != 3 || (LB == 16 && RC == 16), "stage c reads what its own half-warp wrote");
             __syncwarp();
             if (active) {
+                float a0[32];
+                sink.preload(st, a0);   // first half of my accumulators, in flight during the butterfly
                 cpx v[RC];
 #pragma unroll
                 for (int r = 0; r < RC; r++) v[r] = f4_to_cpx(smem[addr(t * RC + r)]);
                 dft<RC>(v);
-                sink.put16(st, m, 0, t, 0, 1, v);
+                sink.put16_preloaded(st, a0, v);
             }
         }
         m += mstride;
