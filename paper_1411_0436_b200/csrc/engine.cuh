@@ -160,7 +160,7 @@ struct SinkStokes {
         u64 pw[16];
         float cr[16], ci[16];
     };
-    __device__ __forceinline__ void init(State&, uint32_t) const {}
+    __device__ __forceinline__ void init(State&, uint32_t, int = 64) const {}
     __device__ __forceinline__ void begin(State& s) const {
 #pragma unroll
         for (int i = 0; i < 16; i++) { s.pw[i] = 0ull; s.cr[i] = 0.f; s.ci[i] = 0.f; }
@@ -340,7 +340,7 @@ struct SinkZ {
     static constexpr bool kAccumulates = false;
     static constexpr bool kTmem = false;
     struct State {};
-    __device__ __forceinline__ void init(State&, uint32_t) const {}
+    __device__ __forceinline__ void init(State&, uint32_t, int = 64) const {}
     __device__ __forceinline__ void begin(State&) const {}
     __device__ __forceinline__ void put16(State&, long long m, int n2, int i, int k0, int ks, const cpx* v) const {
 #pragma unroll
@@ -407,13 +407,52 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
 
     // TMEM accumulators (SinkStokesTmem): 64 columns per warp-quarter set; needs warp-uniform control
     // flow around the tcgen05 instructions, i.e. at least one warp per slot
-    constexpr int TCOLS = (NTS * G > 128) ? 128 : 64;
+    // With the TMEM sink the stage twiddles of the thread (the same for every job) are parked in TMEM
+    // too: columns 64.. of its lane, one tcgen05.ld per stage instead of up to 30 table loads per job.
+    constexpr int TCOLS = (NTS * G > 128) ? 256 : 128;
+    constexpr int TWA = (NST >= 2) ? (16 / RA) * (RA - 1) : 0;       // float2 per thread, stage a
+    constexpr int TWB = (NST == 3) ? (16 / RB) * (RB - 1) : 0;       // stage b
     static_assert(!Sink::kTmem || NTS >= 32, "TMEM sink: a slot must be at least one warp");
+    static_assert(TWA <= 16 && TWB <= 16, "32 words per stage");
     uint32_t tmem_base = 0;
     if (Sink::kTmem) tmem_base = tmem_alloc_cta<TCOLS>((uint32_t*)(bar + 1));
     typename Sink::State st;
-    sink.init(st, tmem_base);
+    sink.init(st, tmem_base, 128);
     sink.begin(st);
+    uint32_t ttw = 0;
+    if (Sink::kTmem) {
+        const int warp = tid >> 5;
+        ttw = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * 128) + 64;
+        float w[32];
+#pragma unroll
+        for (int i = 0; i < 32; i++) w[i] = 0.f;
+#pragma unroll
+        for (int u = 0; u < 16 / RA; u++)
+#pragma unroll
+            for (int q = 1; q < RA; q++) {
+                if (NST >= 2) {
+                    const float2 x = __ldg(twL + (q - 1) * LA + t + NTS * u);
+                    w[2 * (u * (RA - 1) + q - 1)] = x.x;
+                    w[2 * (u * (RA - 1) + q - 1) + 1] = x.y;
+                }
+            }
+        tmem_st32(ttw, w);
+        if (NST == 3) {
+            float w2[32];
+#pragma unroll
+            for (int i = 0; i < 32; i++) w2[i] = 0.f;
+#pragma unroll
+            for (int u = 0; u < 16 / RB; u++)
+#pragma unroll
+                for (int q = 1; q < RB; q++) {
+                    const float2 x = __ldg(twL + (RA - 1) * LA + (q - 1) * LB + (t + NTS * u) % LB);
+                    w2[2 * (u * (RB - 1) + q - 1)] = x.x;
+                    w2[2 * (u * (RB - 1) + q - 1) + 1] = x.y;
+                }
+            tmem_st32(ttw + 32, w2);
+        }
+        tmem_wait_st();
+    }
     // accumulation window of the current job and the job index at which the next window starts:
     // a run that crosses a window boundary flushes its partial sums there and starts over
     long long wcur = (jm.c0 + j0) / jm.M;
@@ -457,6 +496,8 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
         }
         // ---------------- stage a
         if (active) {
+            float twa[32];
+            if (Sink::kTmem && NST >= 2) { tmem_ld32(ttw, twa); tmem_wait_ld(); }
 #pragma unroll
             for (int u = 0; u < 16 / RA; u++) {
                 const int ja = t + NTS * u;
@@ -472,7 +513,9 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                     smem[addr(ja)] = cpx_to_f4(v[0]);
 #pragma unroll
                     for (int q = 1; q < RA; q++) {
-                        const float2 w = __ldg(twL + (q - 1) * LA + ja);  // W_L^{ja q}, table [q][ja]
+                        float2 w;
+                        if (Sink::kTmem) w = make_float2(twa[2 * (u * (RA - 1) + q - 1)], twa[2 * (u * (RA - 1) + q - 1) + 1]);
+                        else w = __ldg(twL + (q - 1) * LA + ja);  // W_L^{ja q}, table [q][ja]
                         smem[addr(ja + q * LA)] = cpx_to_f4(cmul(v[q], w.x, w.y));
                     }
                 }
@@ -483,6 +526,8 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
             if (BULK && tid == 0 && it + 1 < jm.len) issue(it + 1);  // the staging buffer is free again
             // ---------------- stage b
             if (active) {
+                float twb[32];
+                if (Sink::kTmem && NST == 3) { tmem_ld32(ttw + 32, twb); tmem_wait_ld(); }
 #pragma unroll
                 for (int u = 0; u < 16 / RB; u++) {
                     const int i = t + NTS * u;
@@ -498,7 +543,9 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                         smem[addr(base)] = cpx_to_f4(v[0]);
 #pragma unroll
                         for (int q = 1; q < RB; q++) {
-                            const float2 w = __ldg(twL + (RA - 1) * LA + (q - 1) * LB + jb);  // W_LA^{jb q}, table [q][jb]
+                            float2 w;
+                            if (Sink::kTmem) w = make_float2(twb[2 * (u * (RB - 1) + q - 1)], twb[2 * (u * (RB - 1) + q - 1) + 1]);
+                            else w = __ldg(twL + (RA - 1) * LA + (q - 1) * LB + jb);  // W_LA^{jb q}, table [q][jb]
                             smem[addr(base + q * LB)] = cpx_to_f4(cmul(v[q], w.x, w.y));
                         }
                     }
