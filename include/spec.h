@@ -65,7 +65,10 @@ int spec_set_coeffs(spec_t* s, const float* h_coeffs, size_t count);
  * on the concatenated stream, never on how calls split it.  The history starts empty: the first
  * spectrum needs ntaps blocks.  All work is queued on cuda_stream; d_in is borrowed until that
  * work completes.  Returns the number of accumulations completed by this call (>= 0), or
- * SPEC_ERR_SIZE / SPEC_ERR_OVERRUN (nothing queued) / SPEC_ERR_CUDA. */
+ * SPEC_ERR_SIZE / SPEC_ERR_OVERRUN (nothing queued) / SPEC_ERR_CUDA.  The persistent kernel behind
+ * this call bounds every wait it does (about ten seconds); if one ever expires (its grid could not
+ * become resident) the launch ends with invalid sums instead of hanging, and this and every later
+ * spec_process / spec_read_accum on the handle return SPEC_ERR_CUDA until spec_reset. */
 int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* cuda_stream);
 
 /* PAPER.md:95 (step 6).  Pops the oldest completed accumulation into dst as planar

@@ -51,6 +51,8 @@ struct FusedParams {
                            // CTA to leave resets them, so a call needs no memset
     unsigned* a_done;      // [group] finished A tasks          } zeroed before every launch; one counter per
     unsigned* b_done;      // [group] consumed rows (of GS*16)  } GROUP of the launch: no epochs, no divisions
+    unsigned* err;         // mapped host word: set to 1 if a wait inside the kernel timed out (the launch then
+                           // runs to its end with garbage results instead of hanging; the host reports it)
     int dbg_mode;          // timing experiments only (SPEC_FUSED_SKIP): 1 = consumers skip their FFT, 2 = producers skip their work
 };
 
@@ -72,6 +74,27 @@ __device__ __forceinline__ unsigned atom_add_relaxed_u32(unsigned* p, unsigned v
     unsigned r;
     asm volatile("atom.relaxed.gpu.global.add.u32 %0, [%1], %2;" : "=r"(r) : "l"(p), "r"(v) : "memory");
     return r;
+}
+// Bounded wait on a monotonic counter: spins (with back-off) until *ctr >= target, or gives up after about
+// ten seconds and raises the error word.  A wait can only time out if the grid is not fully resident (a
+// foreign kernel holding SM resources for that long) or on a logic error; either way the launch must end.
+__device__ __forceinline__ void wait_counter(const unsigned* ctr, unsigned target, unsigned* err) {
+    if (ld_relaxed_u32(ctr) >= target) return;
+    unsigned long long t0;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    for (unsigned it = 1;; it++) {
+        __nanosleep(200);
+        if (ld_relaxed_u32(ctr) >= target) return;
+        // (the error word lives in host memory: look at it rarely; once it is set everybody drains quickly)
+        if ((it & 0xffffu) == 0 && *(volatile unsigned*)err) return;
+        unsigned long long t1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+        if (t1 - t0 > 10000000000ull) {
+            *(volatile unsigned*)err = 1u;
+            __threadfence_system();
+            return;
+        }
+    }
 }
 __device__ __forceinline__ void red_release_u32(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
@@ -271,7 +294,7 @@ k_fused(const FusedParams p) {
     auto finish = [&]() {
         __syncthreads();
         if (tid == 0) {
-            while (ld_relaxed_u32(p.role + 2) < gridDim.x) __nanosleep(200);
+            wait_counter(p.role + 2, gridDim.x, p.err);
             __threadfence();
             s_role[0] = (atomicAdd(p.role + 3, 1u) == gridDim.x - 1);   // am I the last one out?
         }
@@ -303,7 +326,7 @@ k_fused(const FusedParams p) {
                 asm volatile("cp.async.wait_all;" ::: "memory");
                 if (*(volatile unsigned*)&s_pf[gfree & 3] >= rows_full) return;
             }
-            while (ld_relaxed_u32(p.b_done + gfree) < rows_full) __nanosleep(200);
+            wait_counter(p.b_done + gfree, rows_full, p.err);
         };
         auto prefetch_room = [&](int a) {    // thread 0, for my task a (if any)
             pf_g = -1;
@@ -404,7 +427,7 @@ k_fused(const FusedParams p) {
             if (g != ready_g) {
                 asm volatile("cp.async.wait_all;" ::: "memory");
                 if (*(volatile unsigned*)&s_pf[g & 3] < TPG)
-                    while (ld_relaxed_u32(p.a_done + g) < TPG) __nanosleep(200);
+                    wait_counter(p.a_done + g, TPG, p.err);
                 ready_g = g;
             }
             if (bi + 1 < nbj) {

@@ -64,6 +64,8 @@ struct spec_ctx {
     // fused persistent four-step kernel (fused.cuh)
     bool fused = false;
     int fgrid = 0, fGS = 0, fRING = 0, fna = 2;   // grid, spectra per group, ring groups, producer CTAs per SM
+    unsigned* h_err = nullptr;     // mapped pinned word the fused kernel raises when one of its waits times out
+    unsigned* d_err = nullptr;
     unsigned* d_flags = nullptr;   // [0] next A task, then a_done[fcap], b_done[fcap] (one counter per group of a launch)
     int fcap = 0;
     float* d_ring = nullptr;     // nring accumulators of S*N floats, position order, [pos][S]
@@ -494,6 +496,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     p.N = s->N; p.N2 = s->N2; p.nspec = (int)nspec; p.c0 = c0; p.M = s->M;
     p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / 16); p.na_per_sm = s->fna; p.per_sm = PER_SM;
     p.role = s->d_flags; p.a_done = s->d_flags + FUSED_ROLE_WORDS; p.b_done = s->d_flags + FUSED_ROLE_WORDS + s->fcap;
+    p.err = s->d_err;
     p.dbg_mode = 0;
     if (const char* e = getenv("SPEC_FUSED_SKIP")) p.dbg_mode = atoi(e);
     {
@@ -566,6 +569,7 @@ static void free_all(spec_ctx* s) {
     cudaFree(s->d_coef); cudaFree(s->d_twN); cudaFree(s->d_tw1); cudaFree(s->d_tw2); cudaFree(s->d_perm);
     cudaFree(s->d_hist[0]); cudaFree(s->d_hist[1]); cudaFree(s->d_Z); cudaFree(s->d_ring); cudaFree(s->d_stage);
     cudaFree(s->d_sbuf[0]); cudaFree(s->d_sbuf[1]); cudaFree(s->d_flags);
+    if (s->h_err) cudaFreeHost(s->h_err);
     if (s->side) cudaStreamDestroy(s->side);
     for (int i = 0; i < 2; i++) {
         if (s->ev_copied[i]) cudaEventDestroy(s->ev_copied[i]);
@@ -591,7 +595,12 @@ static int create_impl(spec_ctx* s) {
     // four-step split: one kernel up to 4096 channels, N1 x N2 beyond
     // fused persistent kernel (fused.cuh): dual-pol, 16 x N2, PFB with the paper's 8 taps from 1024
     // channels (the FIR needs the column split to reuse each unpacked sample), direct FFT from 8192
-    s->fused = s->P == 2 && N >= 1024 && N <= 65536 && !getenv("SPEC_NO_FUSED") &&
+    int regs_per_sm = 0, cc_major = 0;
+    CK(cudaDeviceGetAttribute(&regs_per_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev));
+    CK(cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev));
+    // (the resident-grid arithmetic of the fused kernel assumes the 64 K-register SM of sm_100)
+    s->fused = regs_per_sm == 65536 && cc_major == 10 &&
+               s->P == 2 && N >= 1024 && N <= 65536 && !getenv("SPEC_NO_FUSED") &&
                ((s->mode == SPEC_MODE_PFB && s->T == 8) || (s->mode == SPEC_MODE_FFT && N >= 8192));
     if (s->fused) { s->N1 = 16; s->N2 = N / 16; }
     else if (N <= 4096) { s->N1 = 1; s->N2 = N; }
@@ -639,6 +648,9 @@ static int create_impl(spec_ctx* s) {
             s->fRING = a_groups + (int)((b_spectra + s->fGS - 1) / s->fGS) + 2;
             if (const char* e = getenv("SPEC_FUSED_RING")) { const int v = atoi(e); if (v >= 2 && v <= 4096) s->fRING = v; }
             s->zbatch = s->fRING * s->fGS;
+            CK(cudaHostAlloc(&s->h_err, sizeof(unsigned), cudaHostAllocMapped));
+            *s->h_err = 0u;
+            CK(cudaHostGetDevicePointer(&s->d_err, s->h_err, 0));
         }
         CK(cudaMalloc(&s->d_Z, (size_t)s->zbatch * N * sizeof(float4)));
     }
@@ -711,6 +723,10 @@ extern "C" int spec_reset(spec_t* s) {
     if (!s) return SPEC_ERR_ARG;
     CK(cudaDeviceSynchronize());
     s->nhist = 0; s->cur = 0; s->count = 0; s->win_read = 0;
+    if (s->h_err && *s->h_err) {   // a timed-out launch leaves its counters dirty
+        *s->h_err = 0u;
+        if (s->d_flags) CK(cudaMemset(s->d_flags, 0, (size_t)(FUSED_ROLE_WORDS + 2 * s->fcap) * sizeof(unsigned)));
+    }
     CK(cudaMemset(s->d_ring, 0, (size_t)s->nring * acc_floats(s) * sizeof(float)));
     return SPEC_OK;
 }
@@ -722,8 +738,18 @@ extern "C" int spec_set_ring(spec_t* s, int nslots) {
     return alloc_ring(s, nslots);
 }
 
+static int fused_failed(spec_ctx* s) {
+    if (s->h_err && *(volatile unsigned*)s->h_err) {
+        snprintf(g_err, sizeof(g_err), "a wait inside the persistent kernel timed out (grid not fully resident?); "
+                                       "results since the last spec_reset are invalid");
+        return 1;
+    }
+    return 0;
+}
+
 extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* cuda_stream) {
     if (!s) return SPEC_ERR_ARG;
+    if (fused_failed(s)) return SPEC_ERR_CUDA;
     if (nsamples % (size_t)s->N) return SPEC_ERR_SIZE;
     if (nsamples == 0) return 0;
     if (!d_in || ((uintptr_t)d_in & 15)) return SPEC_ERR_ARG;  // bulk copies need 16-byte alignment
@@ -766,6 +792,7 @@ extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* 
 
 extern "C" int spec_read_accum(spec_t* s, float* dst, int dst_is_device, void* cuda_stream) {
     if (!s || !dst) return SPEC_ERR_ARG;
+    if (fused_failed(s)) return SPEC_ERR_CUDA;
     if (windows_done(s) - s->win_read <= 0) return 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     float* acc = s->d_ring + (size_t)(s->win_read % s->nring) * acc_floats(s);
