@@ -632,8 +632,7 @@ static int create_impl(spec_ctx* s) {
             int rc = fused_dispatch(s, true, none, 0, 0, nullptr);
             if (rc) return rc;
             const int NT = (s->N2 == 4096) ? 256 : 128;
-            s->fGS = (s->N2 >= 512) ? 16 : 64;
-            if (N == 65536) s->fGS = 8;
+            s->fGS = (s->N2 >= 512) ? 16 : 32;   // spectra per ring group (measured best: profiles/r01b_tuning.md)
             if (const char* e = getenv("SPEC_FUSED_GS")) { const int v = atoi(e); if (v >= 2 && v <= 4096 && !(v & (v - 1))) s->fGS = v; }
             // producer share of the resident CTAs: the FIR makes an A task about as long as the row FFT of
             // the same samples; without it (direct-FFT mode) one producer feeds three consumers
