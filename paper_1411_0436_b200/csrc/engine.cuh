@@ -142,6 +142,21 @@ struct FrontZ {
     }
 };
 
+// front end for `pass A` behind the stand-alone FIR kernel (k_fir8, passa_pfb.cuh): element e of column
+// `off` of the filtered spectrum Y[m][n] (float4 = Xre,Yre,Xim,Yim), n = e*stride + off
+struct FrontY {
+    const float4* Y;
+    int N, stride;
+    static constexpr bool kBulk = false;
+    static constexpr int kElemBytes = 16;
+    __device__ __forceinline__ const void* src(long long, int) const { return nullptr; }
+    __device__ __forceinline__ cpx decode(const void*, int) const { return {0ull, 0ull}; }
+    __device__ __forceinline__ int off(int slot_id) const { return slot_id; }
+    __device__ __forceinline__ cpx load(long long m, int e, int off_) const {
+        return f4_to_cpx(__ldcg(Y + (size_t)m * N + (size_t)e * stride + off_));
+    }
+};
+
 // ---- sinks
 // The last engine stage hands each sink the 16 outputs of one radix-16 butterfly at once:
 //   put16(state, m, off, i, k0, ks, v): v[q] is the output at engine position p = 16*i + q,

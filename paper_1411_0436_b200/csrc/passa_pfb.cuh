@@ -97,4 +97,41 @@ k_passA_pfb16(const InputView view, const float* __restrict__ h, float4* __restr
     }
 }
 
+// Stand-alone 8-tap polyphase FIR (step 3) for the splits whose first factor is larger than 16
+// (N >= 131072): y[m][n] = sum_t h[tN+n] x[(m+t)N+n] for a chunk of CH consecutive spectra per thread,
+// one filter branch n per thread (coalesced over n), an 8-sample register window that slides by one block
+// per spectrum (every raw sample is loaded and unpacked once per chunk).  Output Y[m][n] as float4
+// (Xre, Yre, Xim, Yim), read back by pass A through FrontY.
+template <int P, int CH>
+__global__ void __launch_bounds__(256)
+k_fir8(const InputView view, const float* __restrict__ h, float4* __restrict__ Y, int N, long long m0, int nb) {
+    constexpr int T = 8;
+    static_assert(CH % T == 0, "chunk is a whole number of window rotations");
+    const int n = blockIdx.x * blockDim.x + threadIdx.x;
+    const int j0 = blockIdx.y * CH;
+    if (n >= N || j0 >= nb) return;
+    const int j1 = (j0 + CH < nb) ? j0 + CH : nb;
+    float hc[T];
+#pragma unroll
+    for (int t = 0; t < T; t++) hc[t] = __ldg(h + (size_t)t * N + n);
+    cpx x[T];
+#pragma unroll
+    for (int t = 0; t < T - 1; t++) x[t] = load_raw<P>(view, m0 + j0 + t, n, N);
+    for (int j = j0; j < j1; j += T) {
+#pragma unroll
+        for (int r = 0; r < T; r++) {
+            if (j + r < j1) {
+                x[(r + T - 1) % T] = load_raw<P>(view, m0 + j + r + T - 1, n, N);
+                u64 re = 0ull, im = 0ull;
+#pragma unroll
+                for (int t = 0; t < T; t++) {
+                    re = fma2(x[(r + t) % T].re, bc(hc[t]), re);
+                    im = fma2(x[(r + t) % T].im, bc(hc[t]), im);
+                }
+                Y[(size_t)(j + r) * N + n] = cpx_to_f4({re, im});
+            }
+        }
+    }
+}
+
 }  // namespace spk

@@ -60,6 +60,7 @@ struct spec_ctx {
     uint8_t* d_hist[2] = {nullptr, nullptr};
     int cur = 0, nhist = 0;
     float4* d_Z = nullptr;       // four-step intermediate, zbatch spectra (fused path: the Z ring)
+    float4* d_Y = nullptr;       // FIR output of a batch (two-launch path with N1 > 16, 8 taps)
     int zbatch = 0;
     // fused persistent four-step kernel (fused.cuh)
     bool fused = false;
@@ -422,9 +423,49 @@ static int launch_passA_pfb16(spec_ctx* s, const InputView& view, long long m0, 
     return 0;
 }
 
+// N1 > 16 with the paper's 8 taps: stand-alone sliding FIR into Y, then the column FFTs read Y
+template <class PL, int P>
+static int launch_passA_fir(spec_ctx* s, const InputView& view, long long m0, int nb, cudaStream_t st) {
+    constexpr int CH = 32;
+    {
+        ProfScope ps(s, 1, st);
+        k_fir8<P, CH><<<dim3(cdiv(s->N, 256), cdiv(nb, CH)), 256, 0, st>>>(view, s->d_coef, s->d_Y, s->N, m0, nb);
+    }
+    CK(cudaGetLastError());
+    constexpr int G = 256 / PL::NTS;
+    const size_t smem = (PL::NST > 1) ? (size_t)G * PL::L * sizeof(float4) : 0;
+    FrontY front{s->d_Y, s->N, s->N2};
+    SinkZ sink{s->d_Z, s->d_twN, s->N, s->N2};
+    const int gx = s->N2 / G;
+    int ny = cdiv((long long)4 * s->numSM, gx);
+    if (ny > nb) ny = nb;
+    const int len = cdiv(nb, ny);
+    ny = cdiv(nb, len);
+    JobMap jm{nb, len, s->N2, 0, 0, 1};
+    auto kern = k_engine<PL, true, G, 1, FrontY, SinkZ>;
+    int rc = prep_smem(kern, smem);
+    if (rc) return rc;
+    {
+        ProfScope ps(s, 1, st);
+        kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw1);
+    }
+    CK(cudaGetLastError());
+    return 0;
+}
+
 static int run_passA(spec_ctx* s, const InputView& v, long long m0, int nb, cudaStream_t st) {
     if (s->mode == SPEC_MODE_PFB && s->N1 == 16 && s->T == 8)
         return (s->P == 2) ? launch_passA_pfb16<2>(s, v, m0, nb, st) : launch_passA_pfb16<1>(s, v, m0, nb, st);
+    if (s->d_Y) {
+        switch (s->N1) {
+#define AF_CASE(LEN, PLX) \
+    case LEN: return (s->P == 2) ? launch_passA_fir<PLX, 2>(s, v, m0, nb, st) : launch_passA_fir<PLX, 1>(s, v, m0, nb, st);
+            AF_CASE(32, PL32)
+            AF_CASE(64, PL64)
+            AF_CASE(128, PL128)
+#undef AF_CASE
+        }
+    }
     switch (s->N1) {
 #define A_CASE(LEN, PLX)                                                        \
     case LEN: {                                                                 \
@@ -567,7 +608,7 @@ static void free_all(spec_ctx* s) {
     prof_fold(s);
     for (auto e : s->pool) cudaEventDestroy(e);
     cudaFree(s->d_coef); cudaFree(s->d_twN); cudaFree(s->d_tw1); cudaFree(s->d_tw2); cudaFree(s->d_perm);
-    cudaFree(s->d_hist[0]); cudaFree(s->d_hist[1]); cudaFree(s->d_Z); cudaFree(s->d_ring); cudaFree(s->d_stage);
+    cudaFree(s->d_hist[0]); cudaFree(s->d_hist[1]); cudaFree(s->d_Z); cudaFree(s->d_Y); cudaFree(s->d_ring); cudaFree(s->d_stage);
     cudaFree(s->d_sbuf[0]); cudaFree(s->d_sbuf[1]); cudaFree(s->d_flags);
     if (s->h_err) cudaFreeHost(s->h_err);
     if (s->side) cudaStreamDestroy(s->side);
@@ -652,6 +693,8 @@ static int create_impl(spec_ctx* s) {
             CK(cudaHostGetDevicePointer(&s->d_err, s->h_err, 0));
         }
         CK(cudaMalloc(&s->d_Z, (size_t)s->zbatch * N * sizeof(float4)));
+        if (!s->fused && s->mode == SPEC_MODE_PFB && s->T == 8 && s->N1 > 16)
+            CK(cudaMalloc(&s->d_Y, (size_t)s->zbatch * N * sizeof(float4)));
     }
     std::vector<int> perm(N);
     for (int a = 0; a < N; a++) {
