@@ -664,7 +664,10 @@ static int create_impl(spec_ctx* s) {
         make_twiddles(N, w);
         CK(cudaMalloc(&s->d_twN, w.size() * sizeof(float2)));
         CK(cudaMemcpy(s->d_twN, w.data(), w.size() * sizeof(float2), cudaMemcpyHostToDevice));
-        size_t zmb = 32;  // intermediate sized to stay L2-resident; SPEC_ZBATCH_MB overrides
+        // two-launch path: the Z batch of one launch pair.  Measured (profiles/r01b_tuning.md): long runs per CTA
+        // and few launches matter more here than keeping Z in L2, so the batch covers a whole 64 MiB call
+        // (256 MiB of Z); SPEC_ZBATCH_MB overrides
+        size_t zmb = 256;
         if (const char* e = getenv("SPEC_ZBATCH_MB")) { const long v = atol(e); if (v >= 1 && v <= 4096) zmb = (size_t)v; }
         size_t zb = (zmb << 20) / ((size_t)N * sizeof(float4));
         s->zbatch = (int)(zb < 1 ? 1 : zb);
