@@ -147,6 +147,35 @@ def test_parity_fused_kernel_ring_wraps(nchan, mode, nspec, M):
         compare(a, b, f"fused ring N={nchan} mode={mode}")
 
 
+def test_two_handles_on_two_streams_share_the_gpu():
+    """Two persistent-kernel handles fed alternately on two CUDA streams: the second launch can only become
+    resident as the first one drains (both size their grid to the whole GPU); results must not depend on it."""
+    torch, sp = _torch(), _sp()
+    cfgs = [(8192, PFB, 8, 40), (32768, FFT, 1, 16)]
+    raws = [synth.dual_pol_stream(900 + i, (3 * M + T - 1) * N, [synth.F_CFG1]) for i, (N, mode, T, M) in enumerate(cfgs)]
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    specs, devs, outs = [], [], [[], []]
+    for (N, mode, T, M), raw in zip(cfgs, raws):
+        specs.append(sp.Spec(N, T, 2, mode, M, 1 if mode == PFB else 0))
+        devs.append(torch.from_numpy(raw.reshape(-1)).cuda())
+    torch.cuda.synchronize()
+    for part in range(3):   # three calls per handle, interleaved
+        for i, ((N, mode, T, M), raw) in enumerate(zip(cfgs, raws)):
+            nblk = raw.shape[0] // N
+            lo = part * nblk // 3
+            hi = (part + 1) * nblk // 3
+            specs[i].process(devs[i].data_ptr() + lo * N * 4, (hi - lo) * N, streams[i].cuda_stream)
+    for i in range(2):
+        while specs[i].pending():
+            outs[i].append(specs[i].read_accum_host(streams[i].cuda_stream))
+        specs[i].close()
+    for i, ((N, mode, T, M), raw) in enumerate(zip(cfgs, raws)):
+        r, _ = oracle_run(raw, N, T, 2, mode, M, window=(1 if mode == PFB else 0))
+        assert len(outs[i]) == len(r) == 3
+        for a, b in zip(outs[i], r):
+            compare(a, b, f"two handles N={N}")
+
+
 @pytest.mark.parametrize("nchan", [131072, 262144, 524288])
 def test_parity_largest_channel_counts(nchan):
     T, M = 8, 2
