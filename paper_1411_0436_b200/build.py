@@ -19,6 +19,7 @@ DEPS = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith(("
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
+    "-split-compile", "0",   # optimise and assemble the kernels in parallel (2.5 min -> 1.4 min on 8 cores)
 ]
 
 
