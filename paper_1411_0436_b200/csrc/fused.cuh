@@ -420,22 +420,29 @@ k_fused(const FusedParams p) {
     long long nextb = 0;       // first spectrum (of this launch) that no longer belongs to window wcur
     int ready_g = -1;          // thread 0: newest group known to be complete
 
-    if (tid == 0 && nbj > 0) prefetch_line(p.a_done + (group_of_job(0) & ~3));
-    for (int bi = 0; bi < nbj; bi++) {
-        if (tid == 0) {
-            const int g = group_of_job(bi);
-            if (g != ready_g) {
-                asm volatile("cp.async.wait_all;" ::: "memory");
-                if (*(volatile unsigned*)&s_pf[g & 3] < TPG)
-                    wait_counter(p.a_done + g, TPG, p.err);
-                ready_g = g;
-            }
-            if (bi + 1 < nbj) {
-                const int g1 = group_of_job(bi + 1);
-                if (g1 != ready_g) prefetch_line(p.a_done + (g1 & ~3));
-            }
+    // CTA-wide synchronisation of a job: ONE barrier (after stage a's exchange stores).  The write-after-
+    // read hazard on the exchange buffer (stage a of job i+1 overwrites what the last stage of job i
+    // reads) is covered by a split-phase mbarrier instead of a second barrier: a thread arrives once its
+    // last butterfly has consumed its loads and only waits just before its next exchange stores, with
+    // the TMEM update, the window check, the row loads and the first butterflies in between.
+    __shared__ uint64_t s_war;
+    if (tid == 0) mbar_init(&s_war, NT);
+    auto wait_ready = [&](int j) {       // thread 0: returns once the group of my job j is complete
+        const int g = group_of_job(j);
+        if (g == ready_g) return;
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        if (*(volatile unsigned*)&s_pf[g & 3] < TPG) wait_counter(p.a_done + g, TPG, p.err);
+        ready_g = g;
+    };
+    auto prefetch_ready = [&](int j) {   // thread 0
+        if (j < nbj) {
+            const int g = group_of_job(j);
+            if (g != ready_g) prefetch_line(p.a_done + (g & ~3));
         }
-        __syncthreads();   // publishes "group complete"; also frees the exchange buffer of the previous job
+    };
+    if (tid == 0 && nbj > 0) { prefetch_ready(0); wait_ready(0); prefetch_ready(1); }
+    __syncthreads();
+    for (int bi = 0; bi < nbj; bi++) {
         // ---------------- B job bi: spectrum m (ring position zpos), row `row`
         const bool active = m < p.nspec && p.dbg_mode != 1;
         if (active && m >= nextb) {   // new accumulation window (warp-uniform: a warp never straddles spectra)
@@ -454,6 +461,7 @@ k_fused(const FusedParams p) {
 #pragma unroll
                 for (int r = 0; r < RA; r++) v[u][r] = f4_to_cpx(__ldcg(zrow + t + NTS * u + r * LA));
             tmem_wait_ld();
+            if (bi > 0) mbar_wait(&s_war, (bi - 1) & 1);   // everybody is done reading the previous job
 #pragma unroll
             for (int u = 0; u < 16 / RA; u++) {
                 const int ja = t + NTS * u;
@@ -464,7 +472,12 @@ k_fused(const FusedParams p) {
                     smem[addr(ja + q * LA)] = cpx_to_f4(cmul(v[u][q], twa[2 * (u * (RA - 1) + q - 1)],
                                                              twa[2 * (u * (RA - 1) + q - 1) + 1]));
             }
+        } else if (bi > 0) {
+            mbar_wait(&s_war, (bi - 1) & 1);
         }
+        // the next job's group must be complete before anybody loads its rows: checked here (the poll
+        // was prefetched a job ago), published by the barrier
+        if (tid == 0 && bi + 1 < nbj) { wait_ready(bi + 1); prefetch_ready(bi + 2); }
         __syncthreads();
         if (tid == 0) {   // my rows of this job are consumed: the producers may reuse the ring slot
             const int s0 = (y + bi * ny) * SPJ;
@@ -484,6 +497,7 @@ k_fused(const FusedParams p) {
                 cpx v[RB];
 #pragma unroll
                 for (int r = 0; r < RB; r++) v[r] = f4_to_cpx(smem[addr(base + r * LB)]);
+                if (NST == 2) mbar_arrive(&s_war);   // (release: my reads of the exchange buffer are done)
                 dft<RB>(v);
                 if (NST == 2) {
                     sink.put16(st, m, 0, i, i, RA, v);
@@ -508,10 +522,12 @@ k_fused(const FusedParams p) {
                 cpx v[RC];
 #pragma unroll
                 for (int r = 0; r < RC; r++) v[r] = f4_to_cpx(smem[addr(t * RC + r)]);
+                mbar_arrive(&s_war);   // (release: my reads of the exchange buffer are done)
                 dft<RC>(v);
                 sink.put16_preloaded(st, a0, v);
             }
         }
+        if (!active) mbar_arrive(&s_war);
         m += mstride;
         zpos += zstride;
         if (zpos >= RS) zpos -= RS;
