@@ -479,6 +479,13 @@ k_fused(const FusedParams p) {
         // was prefetched a job ago), published by the barrier
         if (tid == 0 && bi + 1 < nbj) { wait_ready(bi + 1); prefetch_ready(bi + 2); }
         __syncthreads();
+        // The rows just consumed are dead (their ring slot will be rewritten in full): drop their dirty L2
+        // lines instead of letting them be written back to HBM -- the ring is meant to live in L2 only.
+        if (active) {
+#pragma unroll
+            for (int i = 0; i < (L * 16) / (NTS * 128); i++)
+                asm volatile("discard.global.L2 [%0], 128;" ::"l"(zrow + (t + NTS * i) * 8) : "memory");
+        }
         if (tid == 0) {   // my rows of this job are consumed: the producers may reuse the ring slot
             const int s0 = (y + bi * ny) * SPJ;
             int s1 = s0 + SPJ;
