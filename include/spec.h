@@ -78,6 +78,12 @@ int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* cuda_stream
  * Returns 1, or 0 if nothing is pending. */
 int spec_read_accum(spec_t* s, float* dst, int dst_is_device, void* cuda_stream);
 
+/* PAPER.md:95 (step 6), several at once: pops up to max_count of the oldest completed accumulations
+ * with ONE kernel launch into DEVICE memory d_dst as [count][S][nchan] fp32 (each as spec_read_accum
+ * writes it, oldest first); the copy is only queued on cuda_stream.  Returns the count popped (0 if
+ * nothing is pending).  (An extension: north_star names the single-accumulation call above.) */
+int spec_read_accum_batch(spec_t* s, float* d_dst, int max_count, void* cuda_stream);
+
 /* Frees everything the handle owns (synchronises the device). */
 int spec_destroy(spec_t* s);
 

@@ -27,6 +27,9 @@
 
 namespace spk {
 
+#ifndef SPK_WARP_PRODUCER
+#define SPK_WARP_PRODUCER 0   // PFB producers: warp-autonomous (no CTA barriers); 0 = CTA-wide tasks of 16 columns
+#endif
 constexpr int kFusedRoleWords = 516;   // 4 counters + 512 per-SM arrival counters (keeps what follows 16-byte aligned)
 
 struct FusedParams {
@@ -53,6 +56,9 @@ struct FusedParams {
     unsigned* b_done;      // [group] consumed rows (of GS*16)  } GROUP of the launch: no epochs, no divisions
     unsigned* err;         // mapped host word: set to 1 if a wait inside the kernel timed out (the launch then
                            // runs to its end with garbage results instead of hanging; the host reports it)
+    const uint4* carry_src;  // PFB: the last T-1 blocks of this call's input ...
+    uint4* carry_dst;        // ... are copied into the history buffer of the NEXT call by this launch (16-byte chunks),
+    int carry_chunks;        // so that no copy sits between two launches in the stream (0: the host copies)
     int dbg_mode;          // timing experiments only (SPEC_FUSED_SKIP): 1 = consumers skip their FFT, 2 = producers skip their work
 };
 
@@ -214,6 +220,143 @@ __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4*
     }
 }
 
+// Warp-autonomous producer (PFB mode).  A warp owns CW = 4 adjacent columns n2 (all 16 rows n1: 64 filter
+// branches, two per lane) for R = 8 spectra per phase, so the FIR -> column-FFT hand-off (32 (spectrum,
+// column) pairs, one per lane) stays inside the warp: no CTA-wide barrier anywhere in the producer, warps
+// drift freely.  Warp tasks are 4-column tiles, `wr, wr + NAW, ...`; every finished warp task adds one to
+// a_done[g], so a group is complete at N2/4.  Each warp has its own hand-off buffer (row stride YS = 68
+// float4: the 8 lanes of a quarter-warp, 2 spectra x 4 columns, then hit 8 different 16-byte bank groups),
+// its own staged raw tile and its own landing zone for the prefetched b_done poll.
+template <int NT, int N2>
+struct ProducerPfbWarp {
+    static constexpr int CW = 4, R = 8, T = 8, N = 16 * N2, NW = NT / 32, YS = 68;
+    static constexpr int NBLK = R + T - 1;
+    static constexpr int RAW_WORDS = NBLK * 16 * CW;       // u32 per staged tile (per warp)
+    static constexpr int CHUNKS = RAW_WORDS / 4;           // 16-byte copies per tile: one per (block, row)
+    static constexpr size_t SMEM = (size_t)NW * (R * YS * sizeof(float4) + RAW_WORDS * 4);
+
+    static __device__ __forceinline__ void stage(const FusedParams& p, uint32_t* raww, int lane, int wt, int j0) {
+        const int lgTPW = p.lgTPG + 2;                     // warp tasks per group = N2 / 4
+        const int g = wt >> lgTPW, n2_0 = (wt & ((1 << lgTPW) - 1)) * CW;
+        const int GS = 1 << p.lgGS;
+        const int mg = g << p.lgGS;
+        const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;
+        const int qmax = nsp - 1 - j0 + (T - 1);
+#pragma unroll
+        for (int i = 0; i < (CHUNKS + 31) / 32; i++) {
+            const int c = lane + 32 * i;
+            if (CHUNKS % 32 == 0 || c < CHUNKS) {
+                const int q = c >> 4, n1 = c & 15;
+                const int blk = mg + j0 + (q < qmax ? q : qmax);
+                const uint8_t* base = (blk < p.view.nhist) ? p.view.hist + (size_t)blk * N * 4
+                                                           : p.view.in + (size_t)(blk - p.view.nhist) * N * 4;
+                const uint8_t* src = base + ((size_t)n1 * N2 + n2_0) * 4;
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(raww + c * 4)), "l"(src) : "memory");
+            }
+        }
+    }
+};
+
+template <int NT, int N2>
+__device__ __forceinline__ void fused_producer_pfb_warp(const FusedParams& p, float4* smem, unsigned* s_pfw, int rank, int NA,
+                                                        unsigned rows_full) {
+    typedef ProducerPfbWarp<NT, N2> PP;
+    constexpr int CW = PP::CW, R = PP::R, T = PP::T, N = PP::N, NW = PP::NW, YS = PP::YS;
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    float4* const ysw = smem + w * (R * YS);                                        // [R][YS]: (row n1, column) at n1*4 + col
+    uint32_t* const raww = (uint32_t*)(smem + NW * R * YS) + w * PP::RAW_WORDS;     // [R+7][16][CW]
+    unsigned* const pf = s_pfw + 4 * w;
+    const int GS = 1 << p.lgGS;
+    const int lgTPW = p.lgTPG + 2;
+    const int ngroups = (p.nspec + GS - 1) >> p.lgGS;
+    const int nwt = ngroups << lgTPW;
+    const int NAW = NA * NW;
+    const int fr = lane >> 2, fc = lane & 3;
+    int pf_g = -1;   // lane 0: group whose b_done line was prefetched into pf
+    auto prefetch_room = [&](int wt) {
+        pf_g = -1;
+        if (wt < nwt && (wt >> lgTPW) >= p.RING) {
+            pf_g = (wt >> lgTPW) - p.RING;
+            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(pf)), "l"(p.b_done + (pf_g & ~3)) : "memory");
+        }
+    };
+    auto wait_room = [&](int g) {
+        const int gfree = g - p.RING;
+        if (gfree < 0) return;
+        if (pf_g == gfree) {
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            if (*(volatile unsigned*)&pf[gfree & 3] >= rows_full) return;
+        }
+        wait_counter(p.b_done + gfree, rows_full, p.err);
+    };
+    const int wr = rank * NW + w;
+    if (lane == 0) prefetch_room(wr);
+    if (wr < nwt) PP::stage(p, raww, lane, wr, 0);
+    for (int wt = wr; wt < nwt; wt += NAW) {
+        const int g = wt >> lgTPW;
+        const int n2_0 = (wt & ((1 << lgTPW) - 1)) * CW;
+        const int mg = g << p.lgGS;
+        const int nsp = (p.dbg_mode == 2) ? 0 : ((p.nspec - mg < GS) ? p.nspec - mg : GS);
+        const int n2 = n2_0 + fc;
+        float4* const zg = p.Z + ((size_t)((unsigned)g % (unsigned)p.RING) << p.lgGS) * N + n2;
+        float2 tw[16];
+#pragma unroll
+        for (int k = 1; k < 16; k++) tw[k] = __ldg(p.twN + (size_t)n2 * k);
+        float hc[2][T];
+#pragma unroll
+        for (int i = 0; i < 2; i++) {
+            const int beta = lane + 32 * i;
+            const int nbr = (beta / CW) * N2 + n2_0 + (beta % CW);
+#pragma unroll
+            for (int t = 0; t < T; t++) hc[i][t] = __ldg(p.h + t * N + nbr);
+        }
+        for (int j0 = 0; j0 < nsp; j0 += R) {
+            asm volatile("cp.async.wait_all;" ::: "memory");
+            __syncwarp();   // the staged tile is complete; the previous phase's column FFTs have read ysw
+            // ---------------- FIR phase
+#pragma unroll
+            for (int i = 0; i < 2; i++) {
+                const int beta = lane + 32 * i;
+                cpx x[T];
+#pragma unroll
+                for (int t = 0; t < T - 1; t++) x[t] = unpack_cpx<2>(raww[t * 64 + beta]);
+#pragma unroll
+                for (int r = 0; r < R; r++) {
+                    x[(r + T - 1) % T] = unpack_cpx<2>(raww[(r + T - 1) * 64 + beta]);
+                    u64 re = 0ull, im = 0ull;
+#pragma unroll
+                    for (int t = 0; t < T; t++) {
+                        re = fma2(x[(r + t) % T].re, bc(hc[i][t]), re);
+                        im = fma2(x[(r + t) % T].im, bc(hc[i][t]), im);
+                    }
+                    ysw[r * YS + beta] = cpx_to_f4({re, im});
+                }
+            }
+            if (j0 == 0 && lane == 0) wait_room(g);
+            __syncwarp();   // ysw complete, the raw tile is free again
+            // ---------------- stage the next phase (of this task or of my next task)
+            if (j0 + R < nsp) PP::stage(p, raww, lane, wt, j0 + R);
+            else if (wt + NAW < nwt) PP::stage(p, raww, lane, wt + NAW, 0);
+            // ---------------- column FFT phase
+            if (j0 + fr < nsp) {
+                cpx v[16];
+#pragma unroll
+                for (int n1 = 0; n1 < 16; n1++) v[n1] = f4_to_cpx(ysw[fr * YS + n1 * CW + fc]);
+                dft<16>(v);
+                float4* zp = zg + (size_t)(j0 + fr) * N;
+                zp[0] = cpx_to_f4(v[0]);
+#pragma unroll
+                for (int k = 1; k < 16; k++) zp[k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
+            }
+        }
+        __syncwarp();   // every Z store of the warp task has been issued by its lane
+        if (lane == 0) {
+            red_release_u32(p.a_done + g, 1u);   // the warp's Z stores are ordered before it
+            prefetch_room(wt + NAW);
+        }
+    }
+}
+
 // One A task in direct-FFT mode: no pre-filter, the 16 samples of a column go straight
 // from global memory through the unpack into the butterfly.
 template <int NT, int N2, class WaitRoom>
@@ -265,11 +408,13 @@ k_fused(const FusedParams p) {
     __shared__ int s_role[2];
     __shared__ uint32_t s_tmem;
     __shared__ __align__(16) unsigned s_pf[4];      // landing zone of the prefetched counter line
+    __shared__ __align__(16) unsigned s_pfw[4 * (NT / 32)];   // one per warp (warp-autonomous producers)
 
     const int tid = threadIdx.x;
     const int GS = 1 << p.lgGS;
     const int ngroups = (p.nspec + GS - 1) >> p.lgGS;
     const unsigned TPG = 1u << p.lgTPG;
+    const unsigned a_full = (MODE_PFB && SPK_WARP_PRODUCER) ? TPG * 4u : TPG;   // a_done of a complete group
     const unsigned rows_full = (unsigned)GS * 16u;
 
     // Every CTA allocates its TMEM columns first, producers included: a CTA of a kernel that contains
@@ -287,12 +432,27 @@ k_fused(const FusedParams p) {
         s_role[1] = (int)atomicAdd(p.role + (is_a ? 0 : 1), 1u);
         atomicAdd(p.role + 2, 1u);   // arrivals
     }
+    // the history of the next call (the (T-1)*N samples carried across calls), one chunk per thread
+    for (int i = blockIdx.x * NT + tid; i < p.carry_chunks; i += gridDim.x * NT) p.carry_dst[i] = __ldg(p.carry_src + i);
+    if (p.carry_chunks) __threadfence();
     __syncthreads();
+    // Programmatic dependent launch: the next spec_process call's launch (same stream, launched with
+    // programmatic stream serialisation) may start filling SM slots as soon as EVERY CTA of this grid is
+    // resident and has carried its share of the history; its CTAs then land in the slots this grid's CTAs
+    // free one by one (producers leave first, and the first arrivals on an SM produce), so the next call's
+    // pipeline fills while this call's consumers drain.  The two launches share nothing but the
+    // accumulators (atomic adds): Z ring, counters and history buffers alternate between launches, and
+    // a third launch cannot start before this one is gone (its predecessor is not fully resident until
+    // then: the grid is exactly what the SMs hold).
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // No CTA may leave before every CTA of the grid has arrived: an early exit would free a slot on its
     // SM, a late CTA would land there as a fifth arrival and the per-SM role split would be off.
     const uint32_t tmem_base_ = tmem_base;
     auto finish = [&]() {
         __syncthreads();
+        // (the previous launch, if this one overlapped its tail, has completed long before any CTA gets here;
+        // waiting for it formally keeps completion in stream order)
+        asm volatile("griddepcontrol.wait;" ::: "memory");
         if (tid == 0) {
             wait_counter(p.role + 2, gridDim.x, p.err);
             __threadfence();
@@ -335,7 +495,9 @@ k_fused(const FusedParams p) {
                 prefetch_line(p.b_done + (pf_g & ~3));
             }
         };
-        if (MODE_PFB) {
+        if (MODE_PFB && SPK_WARP_PRODUCER) {
+            fused_producer_pfb_warp<NT, L>(p, smem, s_pfw, rank, NA, rows_full);
+        } else if (MODE_PFB) {
             if (tid == 0) prefetch_room(rank);
             fused_producer_pfb<NT, L>(p, smem, rank, NA, natasks, wait_room, [&](int g, int a_next) {
                 red_release_u32(p.a_done + g, 1u);   // all Z stores of the CTA are ordered before it
@@ -431,7 +593,7 @@ k_fused(const FusedParams p) {
         const int g = group_of_job(j);
         if (g == ready_g) return;
         asm volatile("cp.async.wait_all;" ::: "memory");
-        if (*(volatile unsigned*)&s_pf[g & 3] < TPG) wait_counter(p.a_done + g, TPG, p.err);
+        if (*(volatile unsigned*)&s_pf[g & 3] < a_full) wait_counter(p.a_done + g, a_full, p.err);
         ready_g = g;
     };
     auto prefetch_ready = [&](int j) {   // thread 0

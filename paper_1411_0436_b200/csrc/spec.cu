@@ -67,8 +67,13 @@ struct spec_ctx {
     int fgrid = 0, fGS = 0, fRING = 0, fna = 2;   // grid, spectra per group, ring groups, producer CTAs per SM
     unsigned* h_err = nullptr;     // mapped pinned word the fused kernel raises when one of its waits times out
     unsigned* d_err = nullptr;
-    unsigned* d_flags = nullptr;   // [0] next A task, then a_done[fcap], b_done[fcap] (one counter per group of a launch)
+    unsigned* d_flags = nullptr;   // two sets (alternating launches) of: role words, a_done[fcap], b_done[fcap]
     int fcap = 0;
+    int fpdl = 1;                  // fused launches use programmatic stream serialisation (SPEC_FUSED_PDL=0 turns it off)
+    int fpar = 0;                  // which set of counters / which Z ring the next fused launch uses
+    const uint8_t* carry_src = nullptr;   // history carry the next fused launch performs itself (see spec_process)
+    uint8_t* carry_dst = nullptr;
+    size_t carry_bytes = 0;
     float* d_ring = nullptr;     // nring accumulators of S*N floats, position order, [pos][S]
     int nring = 0;
     float* d_stage = nullptr;    // planar read-out staging, S*N
@@ -200,11 +205,14 @@ static void default_coeffs(const spec_ctx* s, std::vector<float>& h) {
 
 // ------------------------------------------------------------------ small kernels
 // read-out: position order [pos][S] -> planar natural order [S][N]  (PAPER.md:95 step 6)
-__global__ void k_unpermute(float* __restrict__ acc, const int* __restrict__ perm, float* __restrict__ out,
-                            int N, int S) {
+// blockIdx.y = which of the accumulations popped by this launch: ring slot (slot0 + y) % nring -> out + y*S*N
+__global__ void k_unpermute(float* __restrict__ ring, const int* __restrict__ perm, float* __restrict__ dst,
+                            int N, int S, int slot0, int nring) {
     const int a = blockIdx.x * blockDim.x + threadIdx.x;
     if (a >= N) return;
     const int k = perm[a];
+    float* __restrict__ acc = ring + (size_t)((slot0 + blockIdx.y) % nring) * S * N;
+    float* __restrict__ out = dst + (size_t)blockIdx.y * S * N;
     if (S == 4) {
         const float4 v = ((const float4*)acc)[a];
         ((float4*)acc)[a] = make_float4(0.f, 0.f, 0.f, 0.f);   // read and clear: a free ring slot is always zero
@@ -507,7 +515,8 @@ template <class PL, int NT, int MODE_PFB, int PER_SM>
 static int fused_do(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
     auto kern = k_fused<PL, NT, MODE_PFB, PER_SM>;
     // exchange buffer / FIR hand-off, plus (PFB) the staged raw tile of a producer phase: R+7 blocks of 1 KiB
-    const size_t smem = (size_t)NT * 16 * sizeof(float4) + (MODE_PFB ? (size_t)(NT / 16 + 7) * 1024 : 0);
+    size_t smem = (size_t)NT * 16 * sizeof(float4) + (MODE_PFB ? (size_t)(NT / 16 + 7) * 1024 : 0);
+    if (MODE_PFB && SPK_WARP_PRODUCER && ProducerPfbWarp<NT, PL::L>::SMEM > smem) smem = ProducerPfbWarp<NT, PL::L>::SMEM;
     if (query) {
         int rc = prep_smem(kern, smem);
         if (rc) return rc;
@@ -527,22 +536,35 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         s->d_flags = nullptr;
         s->fcap = 0;
         const int cap = (ngroups + ngroups / 2 + 64) & ~3;   // counters are prefetched as 16-byte lines
-        CK(cudaMalloc(&s->d_flags, (size_t)(FUSED_ROLE_WORDS + 2 * cap) * sizeof(unsigned)));
-        CK(cudaMemset(s->d_flags, 0, (size_t)(FUSED_ROLE_WORDS + 2 * cap) * sizeof(unsigned)));   // the kernel leaves them zero
+        CK(cudaMalloc(&s->d_flags, (size_t)2 * (FUSED_ROLE_WORDS + 2 * cap) * sizeof(unsigned)));
+        CK(cudaMemset(s->d_flags, 0, (size_t)2 * (FUSED_ROLE_WORDS + 2 * cap) * sizeof(unsigned)));   // the kernel leaves them zero
         s->fcap = cap;
     }
+    // consecutive launches may overlap (programmatic dependent launch): they alternate between two Z rings
+    // and two sets of counters
+    const int par = s->fpar;
+    s->fpar ^= 1;
+    unsigned* const flags = s->d_flags + (size_t)par * (FUSED_ROLE_WORDS + 2 * s->fcap);
     FusedParams p;
-    p.view = view; p.h = s->d_coef; p.Z = s->d_Z; p.twN = s->d_twN; p.twL = s->d_tw2;
+    p.view = view; p.h = s->d_coef; p.Z = s->d_Z + (size_t)par * s->zbatch * s->N; p.twN = s->d_twN; p.twL = s->d_tw2;
     p.ring = s->d_ring; p.acc_stride = acc_floats(s); p.nring = s->nring;
     p.N = s->N; p.N2 = s->N2; p.nspec = (int)nspec; p.c0 = c0; p.M = s->M;
     p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / 16); p.na_per_sm = s->fna; p.per_sm = PER_SM;
-    p.role = s->d_flags; p.a_done = s->d_flags + FUSED_ROLE_WORDS; p.b_done = s->d_flags + FUSED_ROLE_WORDS + s->fcap;
+    p.role = flags; p.a_done = flags + FUSED_ROLE_WORDS; p.b_done = flags + FUSED_ROLE_WORDS + s->fcap;
     p.err = s->d_err;
+    p.carry_src = (const uint4*)s->carry_src; p.carry_dst = (uint4*)s->carry_dst; p.carry_chunks = (int)(s->carry_bytes / 16);
+    s->carry_bytes = 0;   // (taken)
     p.dbg_mode = 0;
     if (const char* e = getenv("SPEC_FUSED_SKIP")) p.dbg_mode = atoi(e);
     {
         ProfScope ps(s, 0, st);
-        kern<<<dim3(s->fgrid), NT, smem, st>>>(p);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(s->fgrid); cfg.blockDim = dim3(NT); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = at; cfg.numAttrs = s->fpdl ? 1 : 0;
+        CK(cudaLaunchKernelEx(&cfg, kern, p));
     }
     CK(cudaGetLastError());
     if (getenv("SPEC_FUSED_WATCHDOG")) {   // debugging aid: dump the counters if the launch does not finish
@@ -554,7 +576,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
             cudaStream_t side;
             cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking);
             std::vector<unsigned> h((size_t)FUSED_ROLE_WORDS + 2 * s->fcap);
-            cudaMemcpyAsync(h.data(), s->d_flags, h.size() * sizeof(unsigned), cudaMemcpyDeviceToHost, side);
+            cudaMemcpyAsync(h.data(), flags, h.size() * sizeof(unsigned), cudaMemcpyDeviceToHost, side);
             cudaStreamSynchronize(side);
             fprintf(stderr, "[fused HANG] N=%d nspec=%lld grid=%d NT=%d na=%d GS=%d RING=%d ngroups=%d TPG=%d | rankA=%u rankB=%u arrived=%u\n",
                     s->N, nspec, s->fgrid, NT, s->fna, s->fGS, s->fRING, ngroups, s->N2 / 16, h[0], h[1], h[2]);
@@ -695,7 +717,9 @@ static int create_impl(spec_ctx* s) {
             *s->h_err = 0u;
             CK(cudaHostGetDevicePointer(&s->d_err, s->h_err, 0));
         }
-        CK(cudaMalloc(&s->d_Z, (size_t)s->zbatch * N * sizeof(float4)));
+        // (fused path: two rings, alternating launches may overlap)
+        CK(cudaMalloc(&s->d_Z, (size_t)(s->fused ? 2 : 1) * s->zbatch * N * sizeof(float4)));
+        if (const char* e = getenv("SPEC_FUSED_PDL")) s->fpdl = atoi(e);
         if (!s->fused && s->mode == SPEC_MODE_PFB && s->T == 8 && s->N1 > 16)
             CK(cudaMalloc(&s->d_Y, (size_t)s->zbatch * N * sizeof(float4)));
     }
@@ -770,7 +794,7 @@ extern "C" int spec_reset(spec_t* s) {
     s->nhist = 0; s->cur = 0; s->count = 0; s->win_read = 0;
     if (s->h_err && *s->h_err) {   // a timed-out launch leaves its counters dirty
         *s->h_err = 0u;
-        if (s->d_flags) CK(cudaMemset(s->d_flags, 0, (size_t)(FUSED_ROLE_WORDS + 2 * s->fcap) * sizeof(unsigned)));
+        if (s->d_flags) CK(cudaMemset(s->d_flags, 0, (size_t)2 * (FUSED_ROLE_WORDS + 2 * s->fcap) * sizeof(unsigned)));
     }
     CK(cudaMemset(s->d_ring, 0, (size_t)s->nring * acc_floats(s) * sizeof(float)));
     return SPEC_OK;
@@ -809,13 +833,25 @@ extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* 
 
     InputView view{s->d_hist[s->cur], (const uint8_t*)d_in, s->nhist};
     const long long c = s->count + nspec;
-    if (nspec > 0) {
-        int rc = run_spectra(s, view, 0, nspec, s->count, st);
-        if (rc) return rc;
-    }
-    // carry the last min(T-1,total) blocks of  history ++ input  (reading R4)
+    // carry the last min(T-1,total) blocks of  history ++ input  (reading R4).  On the fused path
+    // the launch copies them itself when they all come from this call's input, so that consecutive launches
+    // stay adjacent in the stream (programmatic dependent launch, fused.cuh).
     const long long keep = total < T - 1 ? total : T - 1;
-    if (keep > 0) {
+    bool carried = false;
+    if (nspec > 0) {
+        if (s->fused && s->N1 > 1 && keep > 0 && nblk >= keep && (s->mode == SPEC_MODE_PFB || !s->use_coef)) {
+            const size_t bb = block_bytes(s);
+            s->carry_src = (const uint8_t*)d_in + (size_t)(nblk - keep) * bb;
+            s->carry_dst = s->d_hist[s->cur ^ 1];
+            s->carry_bytes = (size_t)keep * bb;
+            carried = true;
+        }
+        int rc = run_spectra(s, view, 0, nspec, s->count, st);
+        if (rc) { s->carry_bytes = 0; return rc; }
+    }
+    if (carried) {
+        s->cur ^= 1;
+    } else if (keep > 0) {
         const size_t bb = block_bytes(s);
         uint8_t* dst = s->d_hist[s->cur ^ 1];
         const long long first = total - keep;
@@ -840,11 +876,11 @@ extern "C" int spec_read_accum(spec_t* s, float* dst, int dst_is_device, void* c
     if (fused_failed(s)) return SPEC_ERR_CUDA;
     if (windows_done(s) - s->win_read <= 0) return 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    float* acc = s->d_ring + (size_t)(s->win_read % s->nring) * acc_floats(s);
     float* out = dst_is_device ? dst : s->d_stage;
     {
         ProfScope ps(s, 3, st);
-        k_unpermute<<<cdiv(s->N, 256), 256, 0, st>>>(acc, s->d_perm, out, s->N, s->S);
+        k_unpermute<<<cdiv(s->N, 256), 256, 0, st>>>(s->d_ring, s->d_perm, out, s->N, s->S,
+                                                     (int)(s->win_read % s->nring), s->nring);
     }
     CK(cudaGetLastError());
     if (!dst_is_device) {
@@ -853,6 +889,23 @@ extern "C" int spec_read_accum(spec_t* s, float* dst, int dst_is_device, void* c
     }
     s->win_read++;
     return 1;
+}
+
+extern "C" int spec_read_accum_batch(spec_t* s, float* d_dst, int max_count, void* cuda_stream) {
+    if (!s || !d_dst || max_count < 0) return SPEC_ERR_ARG;
+    if (fused_failed(s)) return SPEC_ERR_CUDA;
+    long long n = windows_done(s) - s->win_read;
+    if (n > max_count) n = max_count;
+    if (n <= 0) return 0;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    {
+        ProfScope ps(s, 3, st);
+        k_unpermute<<<dim3(cdiv(s->N, 256), (unsigned)n), 256, 0, st>>>(s->d_ring, s->d_perm, d_dst, s->N, s->S,
+                                                                        (int)(s->win_read % s->nring), s->nring);
+    }
+    CK(cudaGetLastError());
+    s->win_read += n;
+    return (int)n;
 }
 
 extern "C" int spec_stream_host(spec_t* s, const void* h_pinned, size_t nsamples, size_t chunk_samples,

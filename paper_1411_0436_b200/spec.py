@@ -24,7 +24,7 @@ SYMBOLS = [
     "spec_create", "spec_set_coeffs", "spec_process", "spec_read_accum", "spec_destroy",
     "spec_pending", "spec_spectra_done", "spec_reset", "spec_set_ring", "spec_get_coeffs",
     "spec_stream_host", "spec_measure_fp32_peak", "spec_debug_unpack", "spec_debug_fir",
-    "spec_strerror", "spec_last_error", "spec_profile", "spec_profile_read",
+    "spec_strerror", "spec_last_error", "spec_profile", "spec_profile_read", "spec_read_accum_batch",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -38,6 +38,7 @@ _lib.spec_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_int,
 _lib.spec_set_coeffs.argtypes = [_vp, _fp, _sz]
 _lib.spec_process.argtypes = [_vp, _vp, _sz, _vp]
 _lib.spec_read_accum.argtypes = [_vp, _vp, C.c_int, _vp]
+_lib.spec_read_accum_batch.argtypes = [_vp, _vp, C.c_int, _vp]
 _lib.spec_destroy.argtypes = [_vp]
 _lib.spec_pending.argtypes = [_vp]
 _lib.spec_spectra_done.argtypes = [_vp]
@@ -110,6 +111,10 @@ class Spec:
 
     def read_accum_device(self, d_dst_ptr, stream=0):
         return _check(_lib.spec_read_accum(self._h, d_dst_ptr, 1, stream), "spec_read_accum")
+
+    def read_accum_batch_device(self, d_dst_ptr, max_count, stream=0):
+        """Pops up to max_count accumulations into device memory [count][S][nchan]; returns the count."""
+        return _check(_lib.spec_read_accum_batch(self._h, d_dst_ptr, max_count, stream), "spec_read_accum_batch")
 
     def read_accum_host(self, stream=0):
         out = np.empty((self.nstokes, self.nchan), dtype=np.float32)

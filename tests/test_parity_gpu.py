@@ -324,6 +324,33 @@ def test_read_accum_to_device_matches_host():
     compare(outs[1], r[0])
 
 
+def test_read_accum_batch_matches_oracle_across_ring_wrap():
+    """spec_read_accum_batch: several accumulations per launch, oldest first, slots wrapping around the ring."""
+    torch, sp = _torch(), _sp()
+    N, T, M = 2048, 8, 3
+    nblk = 11 * M + T - 1
+    raw = synth.dual_pol_stream(33, nblk * N, [synth.F_CFG1])
+    d = torch.from_numpy(raw.reshape(-1)).cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    s = sp.Spec(N, T, 2, PFB, M)           # default ring: 8 slots
+    o = torch.zeros((8, 4, N), dtype=torch.float32, device="cuda")
+    got = []
+    first = (5 * M + T - 1) * N
+    assert s.process(d.data_ptr(), first, st) == 5
+    assert s.read_accum_batch_device(o.data_ptr(), 4, st) == 4        # max_count honoured
+    got += list(o[:4].cpu().numpy())
+    assert s.pending() == 1
+    assert s.process(d.data_ptr() + first * 4, nblk * N - first, st) == 6   # slots 5,6,7,0,1,2: wraps
+    assert s.read_accum_batch_device(o.data_ptr(), 8, st) == 7
+    got += list(o[:7].cpu().numpy())
+    assert s.read_accum_batch_device(o.data_ptr(), 8, st) == 0
+    s.close()
+    r, _ = oracle_run(raw, N, T, 2, PFB, M)
+    assert len(r) == 11
+    for a, b in zip(got, r):
+        compare(a, b)
+
+
 def test_stream_host_double_buffered_matches_oracle():
     """north_star item (d): pinned host memory, two device buffers, side-stream copies."""
     torch, sp = _torch(), _sp()
