@@ -700,9 +700,11 @@ static int create_impl(spec_ctx* s) {
             const int NT = (s->N2 == 4096) ? 256 : 128;
             s->fGS = (s->N2 >= 512) ? 16 : 32;   // spectra per ring group (measured best: profiles/r01b_tuning.md)
             if (const char* e = getenv("SPEC_FUSED_GS")) { const int v = atoi(e); if (v >= 2 && v <= 4096 && !(v & (v - 1))) s->fGS = v; }
-            // producer share of the resident CTAs: the FIR makes an A task about as long as the row FFT of
-            // the same samples; without it (direct-FFT mode) one producer feeds three consumers
-            s->fna = (NT == 256) ? 1 : ((s->mode == SPEC_MODE_PFB) ? 2 : 1);
+            // producer share of the resident CTAs: two of the four CTAs of an SM produce, in both modes.  The
+            // FIR makes an A task about as long as the row FFT of the same samples; without it (direct-FFT
+            // mode) one producer per SM was the first choice, but two measure faster now that consecutive
+            // launches overlap (profiles/r01e_tuning.md: N=8192 101 -> 115 GHz, N=32768 111 -> 112 GHz)
+            s->fna = (NT == 256) ? 1 : 2;
             if (const char* e = getenv("SPEC_FUSED_NA")) { const int v = atoi(e); if (v >= 1 && v < ((NT == 256) ? 2 : FUSED_PER_SM)) s->fna = v; }
             // ring = what the producers (one task each) and the consumers (one job of 16*NT points each)
             // hold at a time, plus two groups of slack
