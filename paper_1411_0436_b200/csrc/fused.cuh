@@ -531,6 +531,18 @@ k_fused(const FusedParams p) {
     int m = y * SPJ + sub;                          // spectrum of my next job for this slot
     int zpos = m % RS;                              // its ring position
     auto addr = [&](int q) -> int { return slot * L + (q ^ ((q / 16) & 7)); };
+    // The same swizzle written out for the three-stage plans (LA = 256, LB = RB = RC = 16), so that the 16
+    // addresses of a stage are one base plus compile-time offsets plus one of the 8 values (t & 7) ^ k,
+    // instead of 16 independent registers per stage (which ptxas hoists out of the job loop and spills):
+    //   stage a: q = ja + qq*LA, LA % 128 == 0  =>  addr(q) = addr(ja) + qq*LA
+    //   stage b: q = (t/16)*LA + t%16 + 16 r     =>  (q/16) & 7 = r & 7, the XOR touches t%16 only
+    //   stage c: q = 16 t + r                    =>  (q/16) & 7 = t & 7, the XOR touches r only
+    const int c7 = t & 7;
+    const int bbase = slot * L + (t >> 4) * LA + (t & 8);
+    const int cbase = slot * L + 16 * t;
+    auto addr_b = [&](int r) -> int { return bbase + 16 * r + (c7 ^ (r & 7)); };
+    auto addr_c = [&](int r) -> int { return cbase + (r & 8) + (c7 ^ (r & 7)); };
+    constexpr bool kExplicit = (NST == 3) && (LA % 128 == 0) && (LB == 16) && (RB == 16) && (RC == 16);
     auto group_of_job = [&](int j) -> int {
         int s1 = (y + j * ny) * SPJ + SPJ - 1;
         if (s1 > p.nspec - 1) s1 = p.nspec - 1;
@@ -627,12 +639,13 @@ k_fused(const FusedParams p) {
 #pragma unroll
             for (int u = 0; u < 16 / RA; u++) {
                 const int ja = t + NTS * u;
+                const int aja = addr(ja);
                 dft<RA>(v[u]);
-                smem[addr(ja)] = cpx_to_f4(v[u][0]);
+                smem[aja] = cpx_to_f4(v[u][0]);
 #pragma unroll
                 for (int q = 1; q < RA; q++)
-                    smem[addr(ja + q * LA)] = cpx_to_f4(cmul(v[u][q], twa[2 * (u * (RA - 1) + q - 1)],
-                                                             twa[2 * (u * (RA - 1) + q - 1) + 1]));
+                    smem[kExplicit ? aja + q * LA : addr(ja + q * LA)] =
+                        cpx_to_f4(cmul(v[u][q], twa[2 * (u * (RA - 1) + q - 1)], twa[2 * (u * (RA - 1) + q - 1) + 1]));
             }
         } else if (bi > 0) {
             mbar_wait(&s_war, (bi - 1) & 1);
@@ -665,17 +678,17 @@ k_fused(const FusedParams p) {
                 const int base = qa * LA + jb;
                 cpx v[RB];
 #pragma unroll
-                for (int r = 0; r < RB; r++) v[r] = f4_to_cpx(smem[addr(base + r * LB)]);
+                for (int r = 0; r < RB; r++) v[r] = f4_to_cpx(smem[kExplicit ? addr_b(r) : addr(base + r * LB)]);
                 if (NST == 2) mbar_arrive(&s_war);   // (release: my reads of the exchange buffer are done)
                 dft<RB>(v);
                 if (NST == 2) {
                     sink.put16(st, m, 0, i, i, RA, v);
                 } else {
                     if (u == 0) tmem_wait_ld();
-                    smem[addr(base)] = cpx_to_f4(v[0]);
+                    smem[kExplicit ? addr_b(0) : addr(base)] = cpx_to_f4(v[0]);
 #pragma unroll
                     for (int q = 1; q < RB; q++)
-                        smem[addr(base + q * LB)] = cpx_to_f4(cmul(v[q], twb[2 * (u * (RB - 1) + q - 1)],
+                        smem[kExplicit ? addr_b(q) : addr(base + q * LB)] = cpx_to_f4(cmul(v[q], twb[2 * (u * (RB - 1) + q - 1)],
                                                                   twb[2 * (u * (RB - 1) + q - 1) + 1]));
                 }
             }
@@ -690,7 +703,7 @@ k_fused(const FusedParams p) {
                 sink.preload(st, a0);   // first half of my accumulators, in flight during the butterfly
                 cpx v[RC];
 #pragma unroll
-                for (int r = 0; r < RC; r++) v[r] = f4_to_cpx(smem[addr(t * RC + r)]);
+                for (int r = 0; r < RC; r++) v[r] = f4_to_cpx(smem[kExplicit ? addr_c(r) : addr(t * RC + r)]);
                 mbar_arrive(&s_war);   // (release: my reads of the exchange buffer are done)
                 dft<RC>(v);
                 sink.put16_preloaded(st, a0, v);
