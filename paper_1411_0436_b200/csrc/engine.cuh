@@ -419,6 +419,15 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
         const int s = (RL >= 8) ? (p ^ ((p / RL) & 7)) : p;
         return slot * L + s;
     };
+    // The same swizzle written out for the slot-major three-stage plans (LA = 256, LB = RB = RC = 16): the 16
+    // addresses of a stage become one base + compile-time offsets + one of the 8 values (t & 7) ^ k instead of
+    // 16 independent registers per stage (see fused.cuh: ptxas hoists and spills those)
+    constexpr bool kExplicit = !IL && (NST == 3) && (PL::RLAST == 16) && (LA % 128 == 0) && (LB == 16) && (RB == 16) && (RC == 16);
+    const int c7 = t & 7;
+    const int bbase = slot * L + (t >> 4) * LA + (t & 8);
+    const int cbase = slot * L + 16 * t;
+    auto addr_b = [&](int r) -> int { return bbase + 16 * r + (c7 ^ (r & 7)); };   // == addr((t/16)*LA + t%16 + 16 r)
+    auto addr_c = [&](int r) -> int { return cbase + (r & 8) + (c7 ^ (r & 7)); };  // == addr(16 t + r)
 
     // TMEM accumulators (SinkStokesTmem): 64 columns per warp-quarter set; needs warp-uniform control
     // flow around the tcgen05 instructions, i.e. at least one warp per slot
@@ -525,13 +534,14 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
 #pragma unroll
                     sink.put16(st, m, off, ja, 0, 1, v);
                 } else {
-                    smem[addr(ja)] = cpx_to_f4(v[0]);
+                    const int aja = addr(ja);
+                    smem[aja] = cpx_to_f4(v[0]);
 #pragma unroll
                     for (int q = 1; q < RA; q++) {
                         float2 w;
                         if (Sink::kTmem) w = make_float2(twa[2 * (u * (RA - 1) + q - 1)], twa[2 * (u * (RA - 1) + q - 1) + 1]);
                         else w = __ldg(twL + (q - 1) * LA + ja);  // W_L^{ja q}, table [q][ja]
-                        smem[addr(ja + q * LA)] = cpx_to_f4(cmul(v[q], w.x, w.y));
+                        smem[kExplicit ? aja + q * LA : addr(ja + q * LA)] = cpx_to_f4(cmul(v[q], w.x, w.y));
                     }
                 }
             }
@@ -550,18 +560,18 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                     const int base = qa * LA + jb;
                     cpx v[RB];
 #pragma unroll
-                    for (int r = 0; r < RB; r++) v[r] = f4_to_cpx(smem[addr(base + r * LB)]);
+                    for (int r = 0; r < RB; r++) v[r] = f4_to_cpx(smem[kExplicit ? addr_b(r) : addr(base + r * LB)]);
                     dft<RB>(v);
                     if (NST == 2) {  // LB == 1: i == qa, p = qa*RB + q, k = qa + RA*q
                         sink.put16(st, m, off, i, i, RA, v);
                     } else {
-                        smem[addr(base)] = cpx_to_f4(v[0]);
+                        smem[kExplicit ? addr_b(0) : addr(base)] = cpx_to_f4(v[0]);
 #pragma unroll
                         for (int q = 1; q < RB; q++) {
                             float2 w;
                             if (Sink::kTmem) w = make_float2(twb[2 * (u * (RB - 1) + q - 1)], twb[2 * (u * (RB - 1) + q - 1) + 1]);
                             else w = __ldg(twL + (RA - 1) * LA + (q - 1) * LB + jb);  // W_LA^{jb q}, table [q][jb]
-                            smem[addr(base + q * LB)] = cpx_to_f4(cmul(v[q], w.x, w.y));
+                            smem[kExplicit ? addr_b(q) : addr(base + q * LB)] = cpx_to_f4(cmul(v[q], w.x, w.y));
                         }
                     }
                 }
@@ -579,7 +589,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                     const int i = t + NTS * u;  // i = qa*RB + qb
                     cpx v[RC];
 #pragma unroll
-                    for (int r = 0; r < RC; r++) v[r] = f4_to_cpx(smem[addr(i * RC + r)]);
+                    for (int r = 0; r < RC; r++) v[r] = f4_to_cpx(smem[kExplicit ? addr_c(r) : addr(i * RC + r)]);
                     dft<RC>(v);
                     const int qa = i / RB, qb = i % RB;
                     sink.put16(st, m, off, i, qa + RA * qb, RA * RB, v);
