@@ -3,19 +3,26 @@
 
 Metric (BASELINE.json): complex samples/s per polarisation (= per-polarisation bandwidth) in GHz,
 PFB mode by default on configs[1]: dual-pol PFB, N=32768, T=8, M=256, fed in 64 MiB calls that carry
-the 7*N filter history.  One "step" = 4 such calls (2^26 time samples, 256 MiB of int8 input, larger
-than the 126 MB L2) through the whole chain unpack -> FIR -> FFT -> Stokes -> accumulate -> read-out.
+the 7*N filter history.  One "step" = a whole number of passes over a 256 MiB device-resident stream
+(four 64 MiB calls per pass, larger than the 126 MB L2), as many passes as make a step last about
+60 ms, so that the default 20 steps give a timed region of more than a second; every pass goes through
+the whole chain unpack -> FIR -> FFT -> Stokes -> accumulate -> read-out.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
-                  [--nchan N --mode pfb|fft --nacc M]   (other sweep points, same JSON line)
+                  [--nchan N --mode pfb|fft --nacc M]   (another workload, same JSON line)
+  python bench.py --sweep [--sweep-log2 31]             (configs[4]: 20 points, resident and streamed)
 
 `value`  : inputs resident in HBM before the timed region.
 `e2e`    : the same work through spec_stream_host from PINNED HOST memory (H2D inside the timed
            region, double-buffered on a side stream) plus a device-to-host read of every completed
            accumulation.
-`roofline`: dominant kernel's nominal fp32 flops / its CUDA-event time vs the fp32 peak measured in
-           this run (spec_measure_fp32_peak); `roofline_chain` is north_star's whole-chain roofline.
-`cpu_baseline`: the CPU oracle (oracle/, fp64, single thread) timed on a bounded sample.
+`roofline`: dominant kernel's nominal fp32 flops / its time vs the fp32 peak measured in this run
+           (spec_measure_fp32_peak).  Where one kernel is the whole chain its time is taken from the timed
+           pass itself ((step time - read-out kernels) / launches: the launches overlap there, no event sits
+           between them); `frac_event_bracketed` is the same from a second pass with CUDA events around
+           every launch.  `roofline_chain` is north_star's whole-chain roofline.
+`cpu_baseline`: the CPU oracle (oracle/, fp64) timed on a bounded sample, on one core and on all cores
+           (independent stretches of the stream in separate processes).
 `--impl reference` times the oracle alone (the reference arm of this tier).
 Multi-GPU: the path shards over independent streams (one beam per GPU): every rank
 runs its own stream, no data-path collective, "scaling": "weak".
@@ -38,7 +45,8 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 CHUNK_BYTES = 64 << 20      # 64 MiB calls (configs[1])
-CALLS_PER_STEP = 4
+CALLS_PER_PASS = 4          # one pass = the 256 MiB device-resident stream, read out after its 4 calls
+STEP_TARGET_MS = 60.0       # passes per step are chosen so that a step lasts about this long
 NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x lanes x 2 flops x max SM clock
 
 
@@ -57,12 +65,6 @@ def kernel_flops_per_sample(cls, nchan, n1, ntaps, pfb):
     if cls == "passB":
         return 10.0 * math.log2(n2) + 16.0
     return 0.0
-
-
-def four_step_split(nchan):
-    if nchan <= 4096:
-        return 1
-    return 16 if nchan <= 65536 else nchan // 4096
 
 
 def world():
@@ -145,15 +147,15 @@ def workload_from_args(a):
     return dict(pfb=pfb, nchan=nchan, ntaps=ntaps, nacc=nacc, chunk_samples=chunk_samples, name=name)
 
 
-def cpu_baseline(w, budget_s=10.0):
-    """The oracle as it stands, single thread, on a bounded prefix of the same stream."""
+def _oracle_stretch(args):
+    """Times the oracle as it stands on one stretch of the workload stream (runs in a worker process)."""
+    N, T, pfb, nacc, start, budget_s = args
     import oracle
     from paper_1411_0436_b200 import synth
-    N, T = w["nchan"], w["ntaps"]
-    o = oracle.Oracle(N, T, 2, oracle.MODE_PFB if w["pfb"] else oracle.MODE_FFT, w["nacc"],
-                      oracle.WINDOW_HANN if w["pfb"] else oracle.WINDOW_RECT)
+    o = oracle.Oracle(N, T, 2, oracle.MODE_PFB if pfb else oracle.MODE_FFT, nacc,
+                      oracle.WINDOW_HANN if pfb else oracle.WINDOW_RECT)
     blocks_per_call = max(1, (1 << 19) // N)
-    pos, spectra, t_used = 0, 0, 0.0
+    pos, t_used = start, 0.0
     while t_used < budget_s:
         raw = synth.dual_pol_stream(synth.SEED_BASE + 1, blocks_per_call * N, [synth.F_CFG1], start=pos)
         t0 = time.perf_counter()
@@ -164,9 +166,37 @@ def cpu_baseline(w, budget_s=10.0):
             o.read_accum()
     spectra = o.spectra_done()
     o.close()
+    return spectra, pos - start, t_used
+
+
+def cpu_baseline(w, budget_s=10.0, all_cores=True):
+    """The oracle as it stands on a bounded prefix of the same stream: one core, and (all_cores) one independent
+    stretch of the stream per hardware thread in separate processes (the oracle keeps one static table per process)."""
+    N, T = w["nchan"], w["ntaps"]
+    spectra, nsamp, t_used = _oracle_stretch((N, T, w["pfb"], w["nacc"], 0, budget_s))
     ghz = spectra * N / t_used / 1e9
-    return {"value": ghz, "unit": "GHz", "cores": 1, "kind": "oracle",
-            "sample": f"first {pos} time samples ({spectra} spectra) of the workload stream, {t_used:.1f} s of CPU time"}
+    out = {"value": ghz, "unit": "GHz", "cores": 1, "kind": "oracle",
+           "sample": f"first {nsamp} time samples ({spectra} spectra) of the workload stream, {t_used:.1f} s of CPU time"}
+    if all_cores:
+        import concurrent.futures as cf
+        import multiprocessing as mp
+        ncpu = os.cpu_count() or 1
+        try:
+            ncpu = len(os.sched_getaffinity(0))
+        except (AttributeError, OSError):
+            pass
+        stride = 1 << 26    # each worker takes its own stretch of the stream
+        jobs = [(N, T, w["pfb"], w["nacc"], i * stride, budget_s * 0.6) for i in range(ncpu)]
+        t0 = time.perf_counter()
+        with cf.ProcessPoolExecutor(max_workers=ncpu, mp_context=mp.get_context("spawn")) as ex:
+            res = list(ex.map(_oracle_stretch, jobs))
+        wall = time.perf_counter() - t0
+        tot_spectra = sum(r[0] for r in res)
+        tmax = max(r[2] for r in res)
+        out["all_cores"] = {"value": tot_spectra * N / tmax / 1e9, "unit": "GHz", "cores": ncpu, "kind": "oracle",
+                            "sample": f"{ncpu} processes, each {budget_s * 0.6:.0f} s on its own 2^26-sample stretch "
+                                      f"({tot_spectra} spectra in all; slowest worker {tmax:.1f} s, wall {wall:.1f} s)"}
+    return out
 
 
 def run_reference(a):
@@ -176,9 +206,9 @@ def run_reference(a):
     w = workload_from_args(a)
     vals = []
     for _ in range(a.warmup):
-        cpu_baseline(w, budget_s=1.0)
+        cpu_baseline(w, budget_s=1.0, all_cores=False)
     for _ in range(a.steps):
-        vals.append(cpu_baseline(w, budget_s=max(2.0, 40.0 / max(1, a.steps))))
+        vals.append(cpu_baseline(w, budget_s=max(2.0, 40.0 / max(1, a.steps)), all_cores=False))
     v = float(np.mean([x["value"] for x in vals]))
     N = w["nchan"]
     out = {
@@ -193,21 +223,30 @@ def run_reference(a):
     print(json.dumps(out))
 
 
-def run_ours(a):
+def _setup_device():
     import torch
-
-    from paper_1411_0436_b200 import spec as sp
-    from paper_1411_0436_b200 import synth
-
     rank, local_rank, ws = world()
-    dist = None
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
     torch.cuda.set_device(local_rank)
     device = torch.device("cuda", local_rank)
+    dist = None
     if ws > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=device)
+    return torch, rank, local_rank, ws, device, dist
+
+
+def _peaks():
+    ppath = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    return json.load(open(ppath)) if os.path.exists(ppath) else {}
+
+
+def run_ours(a):
+    from paper_1411_0436_b200 import spec as sp
+    from paper_1411_0436_b200 import synth
+
+    torch, rank, local_rank, ws, device, dist = _setup_device()
 
     def barrier():
         torch.cuda.synchronize()
@@ -218,42 +257,54 @@ def run_ours(a):
     w = workload_from_args(a)
     N, T, M, pfb = w["nchan"], w["ntaps"], w["nacc"], w["pfb"]
     cs = w["chunk_samples"]
-    step_samples = cs * CALLS_PER_STEP
-    n1 = four_step_split(N)
+    pass_samples = cs * CALLS_PER_PASS
 
-    # synthetic stream of configs[1] (config-1 generator), one step long, per-rank seed
-    raw = synth.dual_pol_stream(synth.SEED_BASE + 1 + 1000 * rank, step_samples, [synth.F_CFG1])
+    # synthetic stream of configs[1] (config-1 generator), one pass long, per-rank seed
+    raw = synth.dual_pol_stream(synth.SEED_BASE + 1 + 1000 * rank, pass_samples, [synth.F_CFG1])
     h_pinned = torch.from_numpy(raw.reshape(-1)).pin_memory()
     d_in = h_pinned.to(device, non_blocking=False)
     stream = torch.cuda.current_stream().cuda_stream
 
     s = sp.Spec(N, T, 2, sp.MODE_PFB if pfb else sp.MODE_FFT, M, sp.WINDOW_HANN if pfb else sp.WINDOW_RECT)
-    # accumulations are read out once per step (after its CALLS_PER_STEP calls), so that consecutive
-    # spec_process launches stay adjacent in the stream and may overlap
-    ring = max(8, CALLS_PER_STEP * (cs // N // M + 1) + 2)
+    n1, n2, plan_desc = s.plan_info()
+    # accumulations are read out once per pass (after its 4 calls), so that consecutive spec_process launches
+    # stay adjacent in the stream and may overlap
+    ring = max(8, CALLS_PER_PASS * (cs // N // M + 1) + 2)
     s.set_ring(ring)
     d_out = torch.empty((ring, 4, N), dtype=torch.float32, device=device)
     fp32_peak = sp.measure_fp32_peak(stream)
 
-    def step_resident():
+    def pass_resident():
         nout = 0
-        for c in range(CALLS_PER_STEP):
+        for c in range(CALLS_PER_PASS):
             s.process(d_in.data_ptr() + c * cs * 4, cs, stream)
         while s.pending():
             nout += s.read_accum_batch_device(d_out.data_ptr(), ring, stream)
         return nout
 
-    def step_e2e():
+    def pass_e2e():
         nout = 0
-        s.stream_host(h_pinned.data_ptr(), step_samples, cs, stream)
+        s.stream_host(h_pinned.data_ptr(), pass_samples, cs, stream)
         while s.pending():
             s.read_accum_host(stream)
             nout += 1
         return nout
 
-    def timed(fn, steps, warmup, profile):
-        for _ in range(warmup):
+    def one_pass_ms(fn, reps=3):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(reps):
             fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    def timed(fn, passes, steps, warmup, profile):
+        for _ in range(warmup):
+            for _ in range(passes):
+                fn()
         barrier()
         s.profile(profile)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -261,50 +312,63 @@ def run_ours(a):
         e0.record()
         nout = 0
         for _ in range(steps):
-            nout += fn()
+            for _ in range(passes):
+                nout += fn()
         e1.record()
         barrier()
         t1 = time.time()
         ms = max_over_ranks(e0.elapsed_time(e1), dist, device)
         return ms, nout, s.profile_read(), (t0, t1)
 
+    # passes per step: fixed before the timed region from a short calibration (the same on every rank)
+    p_res = max(1, int(math.ceil(STEP_TARGET_MS / max_over_ranks(one_pass_ms(pass_resident), dist, device))))
+    p_e2e = max(1, int(math.ceil(STEP_TARGET_MS / max_over_ranks(one_pass_ms(pass_e2e, 1), dist, device))))
+
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
         time.sleep(0.3)
-    ms, nout, prof0, (t0, t1) = timed(step_resident, a.steps, a.warmup, False)
+    ms, nout, prof0, (t0, t1) = timed(pass_resident, p_res, a.steps, a.warmup, False)
     clocks = sampler.stop(t0, t1) if rank == 0 else None
-    # per-kernel split for the roofline: the same K steps again with every launch bracketed by CUDA
-    # events (kept out of the pass above: the event records themselves cost device time)
-    ms_prof, _, prof, _ = timed(step_resident, a.steps, 1, True)
-    ms_e2e, nout_e2e, prof_e2e, _ = timed(step_e2e, a.steps, max(1, a.warmup // 2), False)
+    # per-kernel split: the same passes again with every launch bracketed by CUDA events (kept out of the pass
+    # above: the event records cost device time and keep consecutive launches from overlapping)
+    prof_steps = max(1, min(a.steps, 4))
+    ms_prof, _, prof, _ = timed(pass_resident, p_res, prof_steps, 1, True)
+    ms_e2e, nout_e2e, prof_e2e, _ = timed(pass_e2e, p_e2e, a.steps, max(1, a.warmup // 2), False)
     s.close()
 
+    step_samples = pass_samples * p_res
     total_samples = step_samples * a.steps * ws
     value = total_samples / (ms * 1e-3) / 1e9
-    e2e = total_samples / (ms_e2e * 1e-3) / 1e9
+    e2e_step_samples = pass_samples * p_e2e
+    e2e = e2e_step_samples * a.steps * ws / (ms_e2e * 1e-3) / 1e9
 
-    # dominant kernel and its roofline (per-launch averages over the timed region)
+    # dominant kernel and its roofline (per-launch averages)
     kern = max(("single", "passA", "passB"), key=lambda k: prof[k][0])
-    k_ms, k_n = prof[kern]
-    fused = (pfb and 1024 <= N <= 65536) or (not pfb and 8192 <= N <= 65536)
-    kern_name = {"single": "k_fused (persistent four-step: unpack+FIR+FFT+Stokes+accumulate)" if fused
-                 else "k_engine (single-CTA unpack+window+FFT+Stokes+accumulate)",
-                 "passA": "four-step pass A", "passB": "four-step pass B"}[kern]
-    flops_total = kernel_flops_per_sample(kern, N, n1, T, pfb) * step_samples * a.steps
-    achieved = flops_total / (k_ms * 1e-3) / 1e12 if k_ms > 0 else None
+    k_ms, k_n = prof[kern]                       # event-bracketed pass (prof_steps steps)
+    launches0 = {k: v[1] for k, v in prof0.items()}   # launch counts of the timed pass
+    kern_name = plan_desc if kern == "single" else f"{kern} of: {plan_desc}"
+    fps = kernel_flops_per_sample(kern, N, n1, T, pfb)
+    frac_bracketed = (fps * step_samples * prof_steps / (k_ms * 1e-3) / 1e12 / fp32_peak) if k_ms > 0 else None
+    readout_ms = prof["readout"][0] / prof_steps * a.steps        # read-out kernels' share of the timed pass
+    one_kernel = (kern == "single")
+    if one_kernel and ms > readout_ms and launches0[kern]:
+        ms_per_launch = (ms - readout_ms) / launches0[kern]
+        achieved = fps * step_samples * a.steps / ((ms - readout_ms) * 1e-3) / 1e12
+        timing = ("timed pass itself: (step time - read-out kernels) / launches; consecutive launches overlap "
+                  "there (programmatic dependent launch), no event sits between them")
+    else:
+        ms_per_launch = k_ms / k_n if k_n else None
+        achieved = frac_bracketed * fp32_peak if frac_bracketed else None
+        timing = "CUDA events around every launch of a second pass over the same steps (several kernels share the step)"
     traffic = None
     tpath = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(tpath):
         traffic = json.load(open(tpath)).get(f"{kern}:{'pfb' if pfb else 'fft'}:{N}")
-    peaks = {}
-    ppath = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(ppath):
-        peaks = json.load(open(ppath))
-    hbm = peaks.get("hbm_gbs", 6650.0)
+    hbm = _peaks().get("hbm_gbs", 6650.0)
     F = chain_flops_per_sample(N, T, pfb)
     roof_ghz = min(hbm / 4.0, fp32_peak * 1e3 / F)
-    launches = sum(v[1] for v in prof0.values())
+    launches = sum(launches0.values())
 
     if rank != 0:
         return
@@ -313,33 +377,30 @@ def run_ours(a):
         "warmup": a.warmup, "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": w["name"], "nchan": N, "ntaps": T, "npol": 2, "nacc": M, "mode": a.mode,
-                   "samples_per_step": step_samples, "calls_per_step": CALLS_PER_STEP,
-                   "cache": "input per step 256 MiB > 126 MB L2 (no flush needed)", "readout": "spec_read_accum_batch after every step (its 4 calls), inside the timed region",
+                   "samples_per_step": step_samples, "calls_per_step": CALLS_PER_PASS * p_res,
+                   "passes_per_step": p_res, "timed_region_s": ms * 1e-3,
+                   "cache": "every pass streams 256 MiB of input > 126 MB L2 (no flush needed)",
+                   "readout": "spec_read_accum_batch after every pass (4 calls), inside the timed region",
+                   "plan": plan_desc,
                    "parallelism": f"replicas x{ws}" if ws > 1 else "single GPU",
                    "paper_context": "GTX TITAN: 1.1 GHz (PFB) / 1.4 GHz (FFT) dual-pol, PAPER.md:7"},
-        "e2e": {"value": e2e, "unit": "GHz", "h2d_bytes_per_step": step_samples * 4,
+        "e2e": {"value": e2e, "unit": "GHz", "h2d_bytes_per_step": e2e_step_samples * 4,
                 "d2h_bytes_per_step": int(nout_e2e / a.steps * 16 * N), "ms_per_step": ms_e2e / a.steps,
-                "h2d_gbs": step_samples * 4 * a.steps / (ms_e2e * 1e-3) / 1e9},
+                "passes_per_step": p_e2e, "h2d_gbs": e2e_step_samples * 4 * a.steps / (ms_e2e * 1e-3) / 1e9},
         "gpu_launches": int(launches),
         "clocks": clocks,
-        "roofline": {"bound": "alu", "kernel": kern, "kernel_name": kern_name, "achieved": achieved, "peak": fp32_peak, "unit": "TFLOP/s",
-                     "frac": (achieved / fp32_peak) if achieved else None, "traffic": traffic,
+        "roofline": {"bound": "alu", "kernel": kern, "kernel_name": kern_name, "achieved": achieved, "peak": fp32_peak,
+                     "unit": "TFLOP/s", "frac": (achieved / fp32_peak) if achieved else None, "traffic": traffic,
                      "traffic_note": "dram bytes read+write per launch from the ncu --set full capture listed in "
                                      "profiles/traffic.json (algorithmic: 4 B per dual-pol sample)",
-                     "algorithmic_bytes_per_launch": 4 * step_samples // CALLS_PER_STEP,
+                     "algorithmic_bytes_per_launch": 4 * cs,
                      "peak_source": "spec_measure_fp32_peak in this run (FFMA chains, all SMs); "
                                     "MEASURED_PEAKS.json has no fp32 figure",
-                     "peak_nominal": NOMINAL_FP32_TFLOPS, "launches": int(k_n),
-                     "ms_per_launch": k_ms / k_n if k_n else None,
-                     "kernel_ms": {k: v[0] for k, v in prof.items()},
-                     "timing": "CUDA events around every launch of a second pass over the same K steps "
-                               f"({ms_prof / a.steps:.3f} ms/step with the events in the stream)",
-                     # consecutive k_fused launches overlap in the un-bracketed stream (programmatic dependent
-                     # launch); the events of the second pass serialise them, so `frac` is the conservative figure.
-                     # Where one kernel is the whole chain, this is the same ratio from the first (timed) pass:
-                     # its total time minus the read-out kernels' time of the second pass
-                     "frac_in_stream": (flops_total / ((ms - prof["readout"][0]) * 1e-3) / 1e12 / fp32_peak)
-                     if (kern == "single" and ms > prof["readout"][0]) else None},
+                     "peak_nominal": NOMINAL_FP32_TFLOPS, "launches": int(launches0[kern]),
+                     "ms_per_launch": ms_per_launch, "timing": timing,
+                     "frac_event_bracketed": frac_bracketed,
+                     "kernel_ms_event_bracketed": {k: v[0] / prof_steps for k, v in prof.items()},
+                     "ms_per_step_event_bracketed": ms_prof / prof_steps},
         "roofline_chain": {"flops_per_sample": F, "hbm_bound_ghz": hbm / 4.0, "fp32_bound_ghz": fp32_peak * 1e3 / F,
                            "roof_ghz": roof_ghz, "frac": value / ws / roof_ghz},
     }
@@ -350,21 +411,104 @@ def run_ours(a):
         dist.destroy_process_group()
 
 
+def run_sweep(a):
+    """configs[4]: N = 2^10 .. 2^19 x {PFB T=8, direct FFT}, dual-pol full Stokes, nacc chosen so that each run
+    processes 2^L time samples of the config-1 generator (L = 31 by default: nacc = 2^31/N, minus 7 for the PFB),
+    once device-resident and once streamed from pinned host memory with double buffering.  The 2^L samples are
+    the 2^26-sample device / pinned buffer fed repeatedly (the 8 GiB stream itself would take minutes to draw)."""
+    from paper_1411_0436_b200 import spec as sp
+    from paper_1411_0436_b200 import synth
+
+    torch, rank, local_rank, ws, device, dist = _setup_device()
+    if rank != 0:
+        return
+    L = a.sweep_log2
+    buf_samples = 1 << min(26, L)
+    reps = (1 << L) // buf_samples
+    cs = CHUNK_BYTES // 4
+    raw = synth.dual_pol_stream(synth.SEED_BASE + 4, buf_samples, [synth.F_CFG1])
+    h_pinned = torch.from_numpy(raw.reshape(-1)).pin_memory()
+    d_in = h_pinned.to(device)
+    stream = torch.cuda.current_stream().cuda_stream
+    fp32_peak = sp.measure_fp32_peak(stream)
+    hbm = _peaks().get("hbm_gbs", 6650.0)
+    rows = []
+    for mode in ("fft", "pfb"):
+        for lg in range(10, 20):
+            N = 1 << lg
+            pfb = mode == "pfb"
+            T = 8 if pfb else 1
+            M = (1 << L) // N - (T - 1)
+            s = sp.Spec(N, T, 2, sp.MODE_PFB if pfb else sp.MODE_FFT, M, sp.WINDOW_HANN if pfb else sp.WINDOW_RECT)
+            d_out = torch.empty((4, N), dtype=torch.float32, device=device)
+
+            def run_resident():
+                done = 0
+                for r in range(reps):
+                    for c in range(buf_samples // cs):
+                        done += s.process(d_in.data_ptr() + c * cs * 4, cs, stream)
+                assert done == 1, done
+                assert s.read_accum_device(d_out.data_ptr(), stream) == 1
+
+            def run_streamed():
+                done = 0
+                for r in range(reps):
+                    done += s.stream_host(h_pinned.data_ptr(), buf_samples, cs, stream)
+                assert done == 1, done
+                assert s.read_accum_host(stream) is not None
+
+            res = {}
+            for name, fn, nrep in (("resident", run_resident, a.sweep_reps), ("streamed", run_streamed, 1)):
+                s.reset(); fn(); s.reset()          # warm-up run
+                times = []
+                for _ in range(nrep):
+                    torch.cuda.synchronize()
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    e0.record(); fn(); e1.record()
+                    torch.cuda.synchronize()
+                    times.append(e0.elapsed_time(e1))
+                    s.reset()
+                res[name] = (1 << L) / (float(np.median(times)) * 1e-3) / 1e9
+            _, _, desc = s.plan_info()
+            s.close()
+            F = chain_flops_per_sample(N, T, pfb)
+            roof = min(hbm / 4.0, fp32_peak * 1e3 / F)
+            row = {"sweep_point": True, "mode": mode, "nchan": N, "ntaps": T, "nacc": M, "samples": 1 << L,
+                   "resident_ghz": res["resident"], "streamed_ghz": res["streamed"],
+                   "streamed_h2d_gbs": res["streamed"] * 4, "roof_ghz": roof, "frac": res["resident"] / roof,
+                   "fp32_peak_tflops": fp32_peak, "plan": desc}
+            rows.append(row)
+            print(json.dumps(row), flush=True)
+    print(f"\n| mode | N | nacc | resident GHz | % of roofline | streamed GHz (host link GB/s) | roofline GHz |")
+    print("|---|---|---|---|---|---|---|")
+    for r in rows:
+        print(f"| {r['mode']} | {r['nchan']} | {r['nacc']} | {r['resident_ghz']:.1f} | {100 * r['frac']:.1f} | "
+              f"{r['streamed_ghz']:.2f} ({r['streamed_h2d_gbs']:.1f}) | {r['roof_ghz']:.0f} |")
+    print(f"\n2^{L} time samples per point (the 2^{min(26, L)}-sample config-1 buffer fed {reps} times), 64 MiB calls; "
+          f"roofline = min(HBM {hbm:.0f} GB/s / 4 B, fp32 {fp32_peak:.1f} TFLOP/s measured in this run / F(N)); "
+          f"resident: median of {a.sweep_reps} runs.")
+
+
 def main():
     p = argparse.ArgumentParser()
     p.add_argument("--gpus", type=int, default=1)
-    p.add_argument("--steps", type=int, default=10)
+    p.add_argument("--steps", type=int, default=20)
     p.add_argument("--warmup", type=int, default=3)
     p.add_argument("--impl", default="ours", choices=["ours", "reference"])
     p.add_argument("--nchan", type=int, default=32768)
     p.add_argument("--mode", default="pfb", choices=["pfb", "fft"])
     p.add_argument("--nacc", type=int, default=0)
     p.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    p.add_argument("--sweep", action="store_true", help="configs[4]: all 20 points, resident and streamed")
+    p.add_argument("--sweep-log2", type=int, default=31, help="log2 of the time samples per sweep point")
+    p.add_argument("--sweep-reps", type=int, default=3)
     a = p.parse_args()
     if a.warmup < 3 and a.impl == "ours":
         a.warmup = 3
     if a.impl == "reference":
         run_reference(a)
+    elif a.sweep:
+        run_sweep(a)
     else:
         run_ours(a)
 

@@ -15,9 +15,12 @@
  *   - out   planar [S][nchan] fp32, S=4: XX, YY, Re(X conj Y), Im(X conj Y); S=1 (npol=1): |X|^2
  *           summed (not averaged) over nacc consecutive spectra counted from stream start
  *           (PAPER.md:83,94).
- * Every function returns an int: >= 0 success, < 0 an SPEC_ERR_* code; on error the handle's
- * state is unchanged.  No exceptions, no abort.  All calls on one handle come from one host
- * thread.  Device pointers are plain CUDA device pointers; `cuda_stream` is a cudaStream_t
+ * Every function returns an int: >= 0 success, < 0 an SPEC_ERR_* code.  SPEC_ERR_ARG / _STATE / _SIZE /
+ * _OVERRUN are detected before anything is queued and leave the handle's state unchanged.  SPEC_ERR_CUDA /
+ * _NOMEM from spec_process or spec_stream_host mean a CUDA call failed after work had been queued: the
+ * accumulators may be partly updated, the handle is marked failed and every later spec_process /
+ * spec_read_accum returns SPEC_ERR_CUDA until spec_reset.  No exceptions, no abort.  All calls on one handle
+ * come from one host thread.  Device pointers are plain CUDA device pointers; `cuda_stream` is a cudaStream_t
  * passed as void* (NULL = the legacy default stream).  The library never falls back to the CPU:
  * without a CUDA device spec_create fails with SPEC_ERR_CUDA.
  */
@@ -65,8 +68,12 @@ int spec_set_coeffs(spec_t* s, const float* h_coeffs, size_t count);
  * on the concatenated stream, never on how calls split it.  The history starts empty: the first
  * spectrum needs ntaps blocks.  All work is queued on cuda_stream; d_in is borrowed until that
  * work completes.  Returns the number of accumulations completed by this call (>= 0), or
- * SPEC_ERR_SIZE / SPEC_ERR_OVERRUN (nothing queued) / SPEC_ERR_CUDA.  The persistent kernel behind
- * this call bounds every wait it does (about ten seconds); if one ever expires (its grid could not
+ * SPEC_ERR_SIZE / SPEC_ERR_OVERRUN (nothing queued) / SPEC_ERR_CUDA.  No host synchronisation and no
+ * allocation happens in this call (for calls of up to 2^28 samples), so it may be captured into a CUDA graph.
+ * The persistent kernel behind this call (dual-pol, 1024 <= nchan <= 65536) sizes its grid to exactly what the
+ * GPU holds at once (4, or 2, CTAs per SM on every SM) and its CTAs wait for one another: it assumes the
+ * whole GPU is available to it (no MPS / green-context SM limit, no other kernel holding SM resources for
+ * seconds).  Every wait in it is bounded (about ten seconds); if one ever expires (the grid could not
  * become resident) the launch ends with invalid sums instead of hanging, and this and every later
  * spec_process / spec_read_accum on the handle return SPEC_ERR_CUDA until spec_reset. */
 int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* cuda_stream);
@@ -124,12 +131,23 @@ int spec_profile(spec_t* s, int enable);
 int spec_profile_read(spec_t* s, double ms[4], long launches[4]);
 
 /* Test hooks for the bit-exact stages (north_star: "unpack and indexing stages must be bit-exact"):
- * spec_debug_unpack: d_out[i] = float(int8 d_bytes[i]) for i < nbytes, using the hot path's unpack.
- * spec_debug_fir: runs the hot path's front end (unpack + FIR, or unpack + window) for ONE
- * spectrum from d_blocks (ntaps consecutive blocks, device) and writes y as [nchan][2*npol] fp32
- * (re,im per pol) to d_out (device). */
-int spec_debug_unpack(const void* d_bytes, size_t nbytes, float* d_out, void* cuda_stream);
-int spec_debug_fir(spec_t* s, const void* d_blocks, float* d_out, void* cuda_stream);
+ * spec_debug_unpack: d_out[i] = float(int8 d_bytes[i]) for i < nbytes (device pointers), through the unpack
+ * routine the kernels call (npol = 2: the packed dual-pol form, npol = 1: the single-pol form).
+ * spec_debug_fir: runs the FRONT END of the very kernel this handle's plan uses (a DUMP instantiation of the
+ * same kernel template: its staging, index arithmetic, unpack and FIR / window code) on nspec spectra taken
+ * from d_blocks (nspec + ntaps - 1 consecutive blocks, device, 16-byte aligned, history empty) and writes what
+ * it hands to the first butterfly as [nspec][nchan][2*npol] fp32 (re,im per pol) to d_out (device).  The
+ * handle's stream state (history, accumulators, counters) is not touched. */
+int spec_debug_unpack(const void* d_bytes, size_t nbytes, int npol, float* d_out, void* cuda_stream);
+int spec_debug_fir(spec_t* s, const void* d_blocks, int nspec, float* d_out, void* cuda_stream);
+
+/* Test hook for the soak test: a foreign kernel of one CTA per SM that holds smem_bytes of shared memory
+ * (up to 227 KiB) and spins for about ms milliseconds (at most 2000) on cuda_stream. */
+int spec_debug_hog(int ms, size_t smem_bytes, void* cuda_stream);
+
+/* Which kernels the handle's plan uses: the four-step split nchan = n1 * n2 (n1 = 1: one kernel per call, no
+ * split) and a one-line description (kernel template, grid, ring) for reports.  Any pointer may be NULL. */
+int spec_plan_info(const spec_t* s, int* n1, int* n2, char* desc, size_t desc_len);
 
 const char* spec_strerror(int code);
 const char* spec_last_error(void); /* detail of the last SPEC_ERR_CUDA / SPEC_ERR_NOMEM on this thread */

@@ -100,6 +100,13 @@ struct FrontRaw {
         return v;
     }
     __device__ __forceinline__ int off(int slot_id) const { return stride == 1 ? 0 : slot_id; }
+    // test hook (k_engine DUMP): element e of spectrum `job` as the caller's [job][n][re,im per pol]
+    __device__ __forceinline__ void dump_put(float* dump, long long job, int e, int off_, cpx v) const {
+        const size_t o = (size_t)job * N + (size_t)e * stride + off_;
+        const float4 z = cpx_to_f4(v);   // (Xre, Yre, Xim, Yim)
+        if (P == 2) ((float4*)dump)[o] = make_float4(z.x, z.z, z.y, z.w);
+        else ((float2*)dump)[o] = make_float2(z.x, z.z);
+    }
     __device__ __forceinline__ cpx load(long long job, int e, int off_) const {
         const int n = e * stride + off_;
         const long long m = m0 + job;
@@ -136,6 +143,7 @@ struct FrontZ {
     }
     __device__ __forceinline__ cpx decode(const void* x, int e) const { return f4_to_cpx(((const float4*)x)[e]); }
     __device__ __forceinline__ int off(int slot_id) const { return slot_id; }
+    __device__ __forceinline__ void dump_put(float*, long long, int, int, cpx) const {}
     __device__ __forceinline__ cpx load(long long m, int e, int row) const {
         const float4 z = Z[(size_t)m * N + (size_t)row * N2 + e];
         return {pk(z.x, z.y), pk(z.z, z.w)};
@@ -152,6 +160,7 @@ struct FrontY {
     __device__ __forceinline__ const void* src(long long, int) const { return nullptr; }
     __device__ __forceinline__ cpx decode(const void*, int) const { return {0ull, 0ull}; }
     __device__ __forceinline__ int off(int slot_id) const { return slot_id; }
+    __device__ __forceinline__ void dump_put(float*, long long, int, int, cpx) const {}
     __device__ __forceinline__ cpx load(long long m, int e, int off_) const {
         return f4_to_cpx(__ldcg(Y + (size_t)m * N + (size_t)e * stride + off_));
     }
@@ -390,9 +399,11 @@ struct JobMap {
 //   IL = false ("slot-major"): tid -> slot = tid / NTS, t = tid % NTS; A[p] at slot*L + swz(p)
 //   IL = true  ("interleaved", pass A): slot = tid % G, t = tid / G; A[p] at p*G + slot, so that
 //        adjacent lanes are adjacent columns n2 (coalesced input rows and Z rows, no bank conflicts)
-template <class PL, bool IL, int G, int MINB, class Front, class Sink>
+//   DUMP (test hook for the bit-exact stage tests): stage a writes what the front end delivered (unpacked
+//        samples / FIR outputs / windowed samples) to `dump` as [job][n][re,im per pol] and nothing else runs
+template <class PL, bool IL, int G, int MINB, class Front, class Sink, bool DUMP = false>
 __global__ void __launch_bounds__(PL::NTS * G, MINB)
-k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __restrict__ twL) {
+k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __restrict__ twL, float* __restrict__ dump) {
     constexpr int L = PL::L, RA = PL::RA, RB = PL::RB, RC = PL::RC, NST = PL::NST;
     constexpr int LA = PL::LA, LB = PL::LB, NTS = PL::NTS;
     extern __shared__ float4 smem[];
@@ -512,7 +523,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
         const long long m = j0 + it;
         const bool active = slot_ok && (m < j1);
         if (BULK) mbar_wait(bar, it & 1);
-        if (Sink::kAccumulates && active && m == nextb) {
+        if (Sink::kAccumulates && !DUMP && active && m == nextb) {
             flush_all(wcur);
             sink.begin(st);
             wcur++;
@@ -529,9 +540,13 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
 #pragma unroll
                 for (int r = 0; r < RA; r++)
                     v[r] = BULK ? front.decode(xbuf + (size_t)slot * XB, ja + r * LA) : front.load(m, ja + r * LA, off);
+                if (DUMP) {
+#pragma unroll
+                    for (int r = 0; r < RA; r++) front.dump_put(dump, m, ja + r * LA, off, v[r]);
+                    continue;
+                }
                 dft<RA>(v);
                 if (NST == 1) {
-#pragma unroll
                     sink.put16(st, m, off, ja, 0, 1, v);
                 } else {
                     const int aja = addr(ja);
@@ -550,7 +565,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
             __syncthreads();
             if (BULK && tid == 0 && it + 1 < jm.len) issue(it + 1);  // the staging buffer is free again
             // ---------------- stage b
-            if (active) {
+            if (active && !DUMP) {
                 float twb[32];
                 if (Sink::kTmem && NST == 3) { tmem_ld32(ttw + 32, twb); tmem_wait_ld(); }
 #pragma unroll
@@ -583,7 +598,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
         }
         if (NST == 3) {
             // ---------------- stage c
-            if (active) {
+            if (active && !DUMP) {
 #pragma unroll
                 for (int u = 0; u < 16 / RC; u++) {
                     const int i = t + NTS * u;  // i = qa*RB + qb
@@ -599,7 +614,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
         }
     }
 
-    if (Sink::kAccumulates && slot_ok && j0 < j1) flush_all(wcur);
+    if (Sink::kAccumulates && !DUMP && slot_ok && j0 < j1) flush_all(wcur);
     if (Sink::kTmem) tmem_free_cta<TCOLS>(tmem_base);
 }
 

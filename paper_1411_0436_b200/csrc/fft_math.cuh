@@ -5,7 +5,7 @@
 // polarization ... complex-valued samples").  cpx.re = (X.re, Y.re), cpx.im = (X.im, Y.im),
 // each half a 64-bit register pair, so one FFMA2/FADD2/FMUL2 (PTX fma/add/mul.rn.f32x2) does
 // the work of two scalar instructions in one issue slot.  Twiddles are scalars; ptxas folds the
-// {c,c} broadcast into the FFMA2 operand (R.F32 modifier), measured in profiles/r01_ubench.md.
+// {c,c} broadcast into the FFMA2 operand (R.F32 modifier).
 //
 // DFT convention (reading R5): X[k] = sum_n x[n] exp(-2 pi i n k / R),
 // forward, unnormalised.  All dft<R>() leave the outputs in natural order in the same array.
@@ -123,7 +123,7 @@ template <> __device__ __forceinline__ void dft<16>(cpx* v) {
 // ---- exact int8 -> fp32 unpack (reading R13).
 // byte b (two's complement) -> float(b), exact for all 256 values: flip the sign bit so the byte
 // is b+128 unsigned, drop it into the low mantissa byte of 2^23 (0x4B000000) and subtract
-// 2^23+128.  PRMT + FADD per component; I2F.S8 runs at 16/clk/SM on sm_100a (profiles/r01_ubench.md).
+// 2^23+128.  PRMT + FADD per component (the conversion instruction I2F runs at a quarter rate).
 __device__ __forceinline__ void unpack4(uint32_t w, float& b0, float& b1, float& b2, float& b3) {
     const uint32_t u = w ^ 0x80808080u;
     b0 = __uint_as_float(__byte_perm(u, 0x4B000000u, 0x7440)) - 8388736.0f;

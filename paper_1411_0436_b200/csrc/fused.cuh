@@ -27,9 +27,6 @@
 
 namespace spk {
 
-#ifndef SPK_WARP_PRODUCER
-#define SPK_WARP_PRODUCER 0   // PFB producers: warp-autonomous (no CTA barriers); 0 = CTA-wide tasks of 16 columns
-#endif
 constexpr int kFusedRoleWords = 516;   // 4 counters + 512 per-SM arrival counters (keeps what follows 16-byte aligned)
 
 struct FusedParams {
@@ -59,18 +56,15 @@ struct FusedParams {
     const uint4* carry_src;  // PFB: the last T-1 blocks of this call's input ...
     uint4* carry_dst;        // ... are copied into the history buffer of the NEXT call by this launch (16-byte chunks),
     int carry_chunks;        // so that no copy sits between two launches in the stream (0: the host copies)
-    int dbg_mode;          // timing experiments only (SPEC_FUSED_SKIP): 1 = consumers skip their FFT, 2 = producers skip their work
+    unsigned* carry_cnt;     // monotonic: every CTA of a carrying launch adds one after its share of the copy (release);
+    unsigned carry_wait;     // a launch whose history was written that way first waits (acquire) for the counter to
+    int carry_wait_on;       // reach carry_wait: consecutive launches overlap, so stream order does not cover it
+    float* dump;             // DUMP instantiation only (test hook): front-end output [spectrum][n][Xre,Xim,Yre,Yim]
 };
 
-__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
-    unsigned v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-// relaxed counter read: the value may be consumed much later (the scheduler prefetches its polls);
-// ordering against the Z traffic comes from the CTA barrier between the poll and the loads (Z is
-// read with ld.global.cg, so no stale L1 line can be hit) -- an acquire load would invalidate the
-// whole L1 of the SM (CCTL.IVALL) on every poll
+// relaxed (strong, gpu-scope) counter read.  The polls are issued one task ahead into a register, so the L2
+// round trip is hidden; the acquire is a separate fence once the value says "ready" (fence_acquire_gpu).
+// Z itself is read with ld.global.cg, so no stale L1 line can be hit.
 __device__ __forceinline__ unsigned ld_relaxed_u32(const unsigned* p) {
     unsigned v;
     asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -104,6 +98,37 @@ __device__ __forceinline__ void wait_counter(const unsigned* ctr, unsigned targe
 }
 __device__ __forceinline__ void red_release_u32(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+// Acquire side of the counter protocol.  The writer publishes with red.release.gpu after a CTA barrier
+// (cumulative over the CTA's stores); the reader's poll is a relaxed (strong) load, made an acquire by this
+// fence, and the CTA barrier that follows extends the ordering to the other threads of the reader.
+#ifndef SPK_ACQ_FENCE
+#define SPK_ACQ_FENCE 1
+#endif
+#ifndef SPK_LEADER_ROT
+#define SPK_LEADER_ROT 0   // 1: the polling / signalling thread of a CTA sits in warp (rank mod warps) instead of warp 0
+#endif
+__device__ __forceinline__ void fence_acquire_gpu() {
+#if SPK_ACQ_FENCE
+    asm volatile("fence.acq_rel.gpu;" ::: "memory");
+#endif
+}
+// wait until a monotonic (wrapping) counter has passed `target`
+__device__ __forceinline__ void wait_counter_wrap(const unsigned* ctr, unsigned target, unsigned* err) {
+    if ((int)(ld_relaxed_u32(ctr) - target) >= 0) return;
+    unsigned long long t0;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    for (;;) {
+        __nanosleep(200);
+        if ((int)(ld_relaxed_u32(ctr) - target) >= 0) return;
+        unsigned long long t1;
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+        if (t1 - t0 > 10000000000ull) {
+            *(volatile unsigned*)err = 1u;
+            __threadfence_system();
+            return;
+        }
+    }
 }
 
 // ---------------------------------------------------------------- A task, PFB mode
@@ -145,9 +170,9 @@ struct ProducerPfb {
 
 // The producer loop of one CTA in PFB mode: tasks rank, rank + NA, ...; `wait_room(g)` (thread 0) returns
 // once the ring slot of group g may be overwritten, `signal(g, next task)` (thread 0) publishes a finished task.
-template <int NT, int N2, class WaitRoom, class Signal>
+template <int NT, int N2, bool DUMP, class WaitRoom, class Signal>
 __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4* smem, int rank, int NA, int natasks,
-                                                   WaitRoom wait_room, Signal signal) {
+                                                   WaitRoom wait_room, Signal signal, int lead = 0) {
     typedef ProducerPfb<NT, N2> PP;
     constexpr int C = PP::C, R = PP::R, T = PP::T, N = PP::N, BPT = PP::BPT;
     float4* const ysm = smem;                                   // [R][16][C] FIR outputs
@@ -162,7 +187,7 @@ __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4*
         const int g = a >> p.lgTPG, tile = a & TPGm;
         const int n2_0 = tile * C;
         const int mg = g << p.lgGS;
-        const int nsp = (p.dbg_mode == 2) ? 0 : ((p.nspec - mg < GS) ? p.nspec - mg : GS);
+        const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;
         const int n2 = n2_0 + fc;
         float4* const zg = p.Z + ((size_t)((unsigned)g % (unsigned)p.RING) << p.lgGS) * N + n2;
         float2 tw[16];
@@ -198,7 +223,7 @@ __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4*
                     ysm[r * 256 + beta] = cpx_to_f4({re, im});
                 }
             }
-            if (j0 == 0 && tid == 0) wait_room(g);
+            if (!DUMP && j0 == 0 && tid == lead) wait_room(g);
             __syncthreads();   // ysm complete, the raw tile is free again
             // ---------------- stage the next phase (of this task or of my next task)
             if (j0 + R < nsp) PP::stage(p, rawsm, g, tile, j0 + R);
@@ -208,159 +233,31 @@ __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4*
                 cpx v[16];
 #pragma unroll
                 for (int n1 = 0; n1 < 16; n1++) v[n1] = f4_to_cpx(ysm[fr * 256 + n1 * C + fc]);
-                dft<16>(v);
-                float4* zp = zg + (size_t)(j0 + fr) * N;
-                zp[0] = cpx_to_f4(v[0]);
+                if (DUMP) {   // test hook: what the column FFT is about to consume, in the caller's layout
+                    float4* dp = (float4*)p.dump + (size_t)(mg + j0 + fr) * N + n2;
 #pragma unroll
-                for (int k = 1; k < 16; k++) zp[k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
+                    for (int n1 = 0; n1 < 16; n1++) {
+                        const float4 z = cpx_to_f4(v[n1]);
+                        dp[n1 * N2] = make_float4(z.x, z.z, z.y, z.w);
+                    }
+                } else {
+                    dft<16>(v);
+                    float4* zp = zg + (size_t)(j0 + fr) * N;
+                    zp[0] = cpx_to_f4(v[0]);
+#pragma unroll
+                    for (int k = 1; k < 16; k++) zp[k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
+                }
             }
         }
         __syncthreads();   // every Z store of the task has been issued by its thread
-        if (tid == 0) signal(g, a + NA);
-    }
-}
-
-// Warp-autonomous producer (PFB mode).  A warp owns CW = 4 adjacent columns n2 (all 16 rows n1: 64 filter
-// branches, two per lane) for R = 8 spectra per phase, so the FIR -> column-FFT hand-off (32 (spectrum,
-// column) pairs, one per lane) stays inside the warp: no CTA-wide barrier anywhere in the producer, warps
-// drift freely.  Warp tasks are 4-column tiles, `wr, wr + NAW, ...`; every finished warp task adds one to
-// a_done[g], so a group is complete at N2/4.  Each warp has its own hand-off buffer (row stride YS = 68
-// float4: the 8 lanes of a quarter-warp, 2 spectra x 4 columns, then hit 8 different 16-byte bank groups),
-// its own staged raw tile and its own landing zone for the prefetched b_done poll.
-template <int NT, int N2>
-struct ProducerPfbWarp {
-    static constexpr int CW = 4, R = 8, T = 8, N = 16 * N2, NW = NT / 32, YS = 68;
-    static constexpr int NBLK = R + T - 1;
-    static constexpr int RAW_WORDS = NBLK * 16 * CW;       // u32 per staged tile (per warp)
-    static constexpr int CHUNKS = RAW_WORDS / 4;           // 16-byte copies per tile: one per (block, row)
-    static constexpr size_t SMEM = (size_t)NW * (R * YS * sizeof(float4) + RAW_WORDS * 4);
-
-    static __device__ __forceinline__ void stage(const FusedParams& p, uint32_t* raww, int lane, int wt, int j0) {
-        const int lgTPW = p.lgTPG + 2;                     // warp tasks per group = N2 / 4
-        const int g = wt >> lgTPW, n2_0 = (wt & ((1 << lgTPW) - 1)) * CW;
-        const int GS = 1 << p.lgGS;
-        const int mg = g << p.lgGS;
-        const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;
-        const int qmax = nsp - 1 - j0 + (T - 1);
-#pragma unroll
-        for (int i = 0; i < (CHUNKS + 31) / 32; i++) {
-            const int c = lane + 32 * i;
-            if (CHUNKS % 32 == 0 || c < CHUNKS) {
-                const int q = c >> 4, n1 = c & 15;
-                const int blk = mg + j0 + (q < qmax ? q : qmax);
-                const uint8_t* base = (blk < p.view.nhist) ? p.view.hist + (size_t)blk * N * 4
-                                                           : p.view.in + (size_t)(blk - p.view.nhist) * N * 4;
-                const uint8_t* src = base + ((size_t)n1 * N2 + n2_0) * 4;
-                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(raww + c * 4)), "l"(src) : "memory");
-            }
-        }
-    }
-};
-
-template <int NT, int N2>
-__device__ __forceinline__ void fused_producer_pfb_warp(const FusedParams& p, float4* smem, unsigned* s_pfw, int rank, int NA,
-                                                        unsigned rows_full) {
-    typedef ProducerPfbWarp<NT, N2> PP;
-    constexpr int CW = PP::CW, R = PP::R, T = PP::T, N = PP::N, NW = PP::NW, YS = PP::YS;
-    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
-    float4* const ysw = smem + w * (R * YS);                                        // [R][YS]: (row n1, column) at n1*4 + col
-    uint32_t* const raww = (uint32_t*)(smem + NW * R * YS) + w * PP::RAW_WORDS;     // [R+7][16][CW]
-    unsigned* const pf = s_pfw + 4 * w;
-    const int GS = 1 << p.lgGS;
-    const int lgTPW = p.lgTPG + 2;
-    const int ngroups = (p.nspec + GS - 1) >> p.lgGS;
-    const int nwt = ngroups << lgTPW;
-    const int NAW = NA * NW;
-    const int fr = lane >> 2, fc = lane & 3;
-    int pf_g = -1;   // lane 0: group whose b_done line was prefetched into pf
-    auto prefetch_room = [&](int wt) {
-        pf_g = -1;
-        if (wt < nwt && (wt >> lgTPW) >= p.RING) {
-            pf_g = (wt >> lgTPW) - p.RING;
-            asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(pf)), "l"(p.b_done + (pf_g & ~3)) : "memory");
-        }
-    };
-    auto wait_room = [&](int g) {
-        const int gfree = g - p.RING;
-        if (gfree < 0) return;
-        if (pf_g == gfree) {
-            asm volatile("cp.async.wait_all;" ::: "memory");
-            if (*(volatile unsigned*)&pf[gfree & 3] >= rows_full) return;
-        }
-        wait_counter(p.b_done + gfree, rows_full, p.err);
-    };
-    const int wr = rank * NW + w;
-    if (lane == 0) prefetch_room(wr);
-    if (wr < nwt) PP::stage(p, raww, lane, wr, 0);
-    for (int wt = wr; wt < nwt; wt += NAW) {
-        const int g = wt >> lgTPW;
-        const int n2_0 = (wt & ((1 << lgTPW) - 1)) * CW;
-        const int mg = g << p.lgGS;
-        const int nsp = (p.dbg_mode == 2) ? 0 : ((p.nspec - mg < GS) ? p.nspec - mg : GS);
-        const int n2 = n2_0 + fc;
-        float4* const zg = p.Z + ((size_t)((unsigned)g % (unsigned)p.RING) << p.lgGS) * N + n2;
-        float2 tw[16];
-#pragma unroll
-        for (int k = 1; k < 16; k++) tw[k] = __ldg(p.twN + (size_t)n2 * k);
-        float hc[2][T];
-#pragma unroll
-        for (int i = 0; i < 2; i++) {
-            const int beta = lane + 32 * i;
-            const int nbr = (beta / CW) * N2 + n2_0 + (beta % CW);
-#pragma unroll
-            for (int t = 0; t < T; t++) hc[i][t] = __ldg(p.h + t * N + nbr);
-        }
-        for (int j0 = 0; j0 < nsp; j0 += R) {
-            asm volatile("cp.async.wait_all;" ::: "memory");
-            __syncwarp();   // the staged tile is complete; the previous phase's column FFTs have read ysw
-            // ---------------- FIR phase
-#pragma unroll
-            for (int i = 0; i < 2; i++) {
-                const int beta = lane + 32 * i;
-                cpx x[T];
-#pragma unroll
-                for (int t = 0; t < T - 1; t++) x[t] = unpack_cpx<2>(raww[t * 64 + beta]);
-#pragma unroll
-                for (int r = 0; r < R; r++) {
-                    x[(r + T - 1) % T] = unpack_cpx<2>(raww[(r + T - 1) * 64 + beta]);
-                    u64 re = 0ull, im = 0ull;
-#pragma unroll
-                    for (int t = 0; t < T; t++) {
-                        re = fma2(x[(r + t) % T].re, bc(hc[i][t]), re);
-                        im = fma2(x[(r + t) % T].im, bc(hc[i][t]), im);
-                    }
-                    ysw[r * YS + beta] = cpx_to_f4({re, im});
-                }
-            }
-            if (j0 == 0 && lane == 0) wait_room(g);
-            __syncwarp();   // ysw complete, the raw tile is free again
-            // ---------------- stage the next phase (of this task or of my next task)
-            if (j0 + R < nsp) PP::stage(p, raww, lane, wt, j0 + R);
-            else if (wt + NAW < nwt) PP::stage(p, raww, lane, wt + NAW, 0);
-            // ---------------- column FFT phase
-            if (j0 + fr < nsp) {
-                cpx v[16];
-#pragma unroll
-                for (int n1 = 0; n1 < 16; n1++) v[n1] = f4_to_cpx(ysw[fr * YS + n1 * CW + fc]);
-                dft<16>(v);
-                float4* zp = zg + (size_t)(j0 + fr) * N;
-                zp[0] = cpx_to_f4(v[0]);
-#pragma unroll
-                for (int k = 1; k < 16; k++) zp[k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
-            }
-        }
-        __syncwarp();   // every Z store of the warp task has been issued by its lane
-        if (lane == 0) {
-            red_release_u32(p.a_done + g, 1u);   // the warp's Z stores are ordered before it
-            prefetch_room(wt + NAW);
-        }
+        if (!DUMP && tid == lead) signal(g, a + NA);
     }
 }
 
 // One A task in direct-FFT mode: no pre-filter, the 16 samples of a column go straight
 // from global memory through the unpack into the butterfly.
-template <int NT, int N2, class WaitRoom>
-__device__ __forceinline__ void fused_task_A_fft(const FusedParams& p, int g, int tile, WaitRoom wait_room) {
+template <int NT, int N2, bool DUMP, class WaitRoom>
+__device__ __forceinline__ void fused_task_A_fft(const FusedParams& p, int g, int tile, WaitRoom wait_room, int lead = 0) {
     constexpr int C = 16, R = NT / C, N = 16 * N2;
     const int tid = threadIdx.x;
     const int GS = 1 << p.lgGS;
@@ -372,7 +269,7 @@ __device__ __forceinline__ void fused_task_A_fft(const FusedParams& p, int g, in
     float2 tw[16];
 #pragma unroll
     for (int k = 1; k < 16; k++) tw[k] = __ldg(p.twN + (size_t)n2 * k);
-    if (tid == 0) wait_room(g);
+    if (!DUMP && tid == lead) wait_room(g);
     __syncthreads();
     for (int j0 = 0; j0 < nsp; j0 += R) {
         if (j0 + fr < nsp) {
@@ -383,18 +280,27 @@ __device__ __forceinline__ void fused_task_A_fft(const FusedParams& p, int g, in
             cpx v[16];
 #pragma unroll
             for (int n1 = 0; n1 < 16; n1++) v[n1] = unpack_cpx<2>(raw[n1]);
-            dft<16>(v);
-            float4* zp = zg + (size_t)(j0 + fr) * N;
-            zp[0] = cpx_to_f4(v[0]);
+            if (DUMP) {   // test hook: the unpacked samples the butterfly is about to consume
+                float4* dp = (float4*)p.dump + (size_t)(mg + j0 + fr) * N + n2;
 #pragma unroll
-            for (int k = 1; k < 16; k++) zp[k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
+                for (int n1 = 0; n1 < 16; n1++) {
+                    const float4 z = cpx_to_f4(v[n1]);
+                    dp[n1 * N2] = make_float4(z.x, z.z, z.y, z.w);
+                }
+            } else {
+                dft<16>(v);
+                float4* zp = zg + (size_t)(j0 + fr) * N;
+                zp[0] = cpx_to_f4(v[0]);
+#pragma unroll
+                for (int k = 1; k < 16; k++) zp[k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
+            }
         }
     }
     __syncthreads();
 }
 
 // ---------------------------------------------------------------- the kernel
-template <class PL, int NT, int MODE_PFB, int PER_SM>
+template <class PL, int NT, int MODE_PFB, int PER_SM, bool DUMP = false>
 __global__ void __launch_bounds__(NT, PER_SM)
 k_fused(const FusedParams p) {
     constexpr int L = PL::L, RA = PL::RA, RB = PL::RB, RC = PL::RC, NST = PL::NST;
@@ -407,16 +313,28 @@ k_fused(const FusedParams p) {
     extern __shared__ float4 smem[];                // G*L float4: B exchange buffer / A FIR hand-off (+ the staged raw tile)
     __shared__ int s_role[2];
     __shared__ uint32_t s_tmem;
-    __shared__ __align__(16) unsigned s_pf[4];      // landing zone of the prefetched counter line
-    __shared__ __align__(16) unsigned s_pfw[4 * (NT / 32)];   // one per warp (warp-autonomous producers)
 
     const int tid = threadIdx.x;
     const int GS = 1 << p.lgGS;
     const int ngroups = (p.nspec + GS - 1) >> p.lgGS;
     const unsigned TPG = 1u << p.lgTPG;
-    const unsigned a_full = (MODE_PFB && SPK_WARP_PRODUCER) ? TPG * 4u : TPG;   // a_done of a complete group
+    const unsigned a_full = TPG;                    // a_done of a complete group
     const unsigned rows_full = (unsigned)GS * 16u;
 
+    if (DUMP) {
+        // Test hook: every CTA runs the producer's front end on the tasks blockIdx.x, blockIdx.x + gridDim.x, ...
+        // and writes what it would hand to the column FFT; no roles, no tensor memory, no counters, and no CTA
+        // waits for another (this instantiation needs fewer registers, so more CTAs than PER_SM may share an SM).
+        const int natasks = ngroups << p.lgTPG;
+        auto no_wait = [](int) {};
+        if (MODE_PFB) {
+            fused_producer_pfb<NT, L, true>(p, smem, (int)blockIdx.x, (int)gridDim.x, natasks, no_wait, [](int, int) {});
+        } else {
+            for (int a = blockIdx.x; a < natasks; a += gridDim.x)
+                fused_task_A_fft<NT, L, true>(p, a >> p.lgTPG, a & (int)(TPG - 1), no_wait);
+        }
+        return;
+    }
     // Every CTA allocates its TMEM columns first, producers included: a CTA of a kernel that contains
     // tcgen05.alloc holds the SM's allocation permit until it relinquishes it, and (measured) no
     // further CTA of the grid is started on that SM before then.
@@ -431,19 +349,30 @@ k_fused(const FusedParams p) {
         s_role[0] = is_a;
         s_role[1] = (int)atomicAdd(p.role + (is_a ? 0 : 1), 1u);
         atomicAdd(p.role + 2, 1u);   // arrivals
+        // The history this launch reads was written by the previous launch's CTAs (the carry below), and the two
+        // launches overlap: acquire it through the carry counter instead of relying on stream order.  (The
+        // counter is complete long before any CTA of this launch starts: the previous launch triggers its
+        // dependents only after every one of its CTAs has signalled.)
+        if (p.carry_wait_on && is_a) {
+            wait_counter_wrap(p.carry_cnt, p.carry_wait, p.err);
+            fence_acquire_gpu();
+        }
     }
-    // the history of the next call (the (T-1)*N samples carried across calls), one chunk per thread
+    // the history of the next call (the (T-1)*N samples carried across calls), one chunk per thread;
+    // it goes to a buffer that neither this launch nor the previous one reads (three buffers rotate)
     for (int i = blockIdx.x * NT + tid; i < p.carry_chunks; i += gridDim.x * NT) p.carry_dst[i] = __ldg(p.carry_src + i);
-    if (p.carry_chunks) __threadfence();
     __syncthreads();
+    if (p.carry_chunks && tid == 0) red_release_u32(p.carry_cnt, 1u);   // (cumulative over the CTA's stores)
     // Programmatic dependent launch: the next spec_process call's launch (same stream, launched with
     // programmatic stream serialisation) may start filling SM slots as soon as EVERY CTA of this grid is
     // resident and has carried its share of the history; its CTAs then land in the slots this grid's CTAs
     // free one by one (producers leave first, and the first arrivals on an SM produce), so the next call's
-    // pipeline fills while this call's consumers drain.  The two launches share nothing but the
-    // accumulators (atomic adds): Z ring, counters and history buffers alternate between launches, and
-    // a third launch cannot start before this one is gone (its predecessor is not fully resident until
-    // then: the grid is exactly what the SMs hold).
+    // pipeline fills while this call's consumers drain.  The two launches share the accumulators (atomic
+    // adds) and the history buffer this launch has just written (acquired by the next launch through
+    // carry_cnt); Z rings and counters alternate between launches, the history rotates through three
+    // buffers (the next launch writes the one neither of the two reads), and a third launch cannot start
+    // before this one is gone (its predecessor is not fully resident until then: the grid is exactly what
+    // the SMs hold).
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // No CTA may leave before every CTA of the grid has arrived: an early exit would free a slot on its
     // SM, a late CTA would land there as a fifth arrival and the per-SM role split would be off.
@@ -468,47 +397,43 @@ k_fused(const FusedParams p) {
     };
     const bool is_a = s_role[0] != 0;
     const int rank = s_role[1];
+    const int lead = SPK_LEADER_ROT ? 32 * (rank % (NT / 32)) : 0;   // the CTA's polling / signalling thread
     const int per_sm = PER_SM;
     const int nsm = (int)gridDim.x / per_sm;
-    auto prefetch_line = [&](const unsigned* src) {
-        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(s_pf)), "l"(src) : "memory");
-    };
+    // thread 0's polls are issued one task ahead into a register (pf_val: the counter of group pf_g)
+    unsigned pf_val = 0u;
+    int pf_g = -1;
 
     if (is_a) {
         // ================= producer: A tasks rank, rank + NA, ...
         const int NA = nsm * p.na_per_sm;
         const int natasks = ngroups << p.lgTPG;
-        int pf_g = -1;   // thread 0: group whose b_done line was prefetched into s_pf
+        int room_g = -1;   // thread 0: newest group whose ring slot is known to be free
         auto wait_room = [&](int g) {
             const int gfree = g - p.RING;     // the group whose ring slot this task overwrites
-            if (gfree < 0) return;
-            if (pf_g == gfree) {
-                asm volatile("cp.async.wait_all;" ::: "memory");
-                if (*(volatile unsigned*)&s_pf[gfree & 3] >= rows_full) return;
-            }
-            wait_counter(p.b_done + gfree, rows_full, p.err);
+            if (gfree < 0 || gfree <= room_g) return;
+            if (!(pf_g == gfree && pf_val >= rows_full)) wait_counter(p.b_done + gfree, rows_full, p.err);
+            fence_acquire_gpu();   // the consumers' reads of the slot happen before my CTA's stores (after the barrier)
+            room_g = gfree;
         };
         auto prefetch_room = [&](int a) {    // thread 0, for my task a (if any)
-            pf_g = -1;
-            if (a < natasks && (a >> p.lgTPG) >= p.RING) {
+            if (a < natasks && (a >> p.lgTPG) >= p.RING && (a >> p.lgTPG) - p.RING > room_g) {
                 pf_g = (a >> p.lgTPG) - p.RING;
-                prefetch_line(p.b_done + (pf_g & ~3));
+                pf_val = ld_relaxed_u32(p.b_done + pf_g);
             }
         };
-        if (MODE_PFB && SPK_WARP_PRODUCER) {
-            fused_producer_pfb_warp<NT, L>(p, smem, s_pfw, rank, NA, rows_full);
-        } else if (MODE_PFB) {
-            if (tid == 0) prefetch_room(rank);
-            fused_producer_pfb<NT, L>(p, smem, rank, NA, natasks, wait_room, [&](int g, int a_next) {
+        if (MODE_PFB) {
+            if (tid == lead) prefetch_room(rank);
+            fused_producer_pfb<NT, L, false>(p, smem, rank, NA, natasks, wait_room, [&](int g, int a_next) {
                 red_release_u32(p.a_done + g, 1u);   // all Z stores of the CTA are ordered before it
                 prefetch_room(a_next);
-            });
+            }, lead);
         } else {
             for (int a = rank; a < natasks; a += NA) {
                 const int g = a >> p.lgTPG;
-                if (tid == 0) prefetch_room(a);
-                fused_task_A_fft<NT, L>(p, g, a & (int)(TPG - 1), wait_room);   // ends with a __syncthreads
-                if (tid == 0) red_release_u32(p.a_done + g, 1u);
+                if (tid == lead) prefetch_room(a);
+                fused_task_A_fft<NT, L, false>(p, g, a & (int)(TPG - 1), wait_room, lead);   // ends with a __syncthreads
+                if (tid == lead) red_release_u32(p.a_done + g, 1u);
             }
         }
         finish();
@@ -604,21 +529,21 @@ k_fused(const FusedParams p) {
     auto wait_ready = [&](int j) {       // thread 0: returns once the group of my job j is complete
         const int g = group_of_job(j);
         if (g == ready_g) return;
-        asm volatile("cp.async.wait_all;" ::: "memory");
-        if (*(volatile unsigned*)&s_pf[g & 3] < a_full) wait_counter(p.a_done + g, a_full, p.err);
+        if (!(pf_g == g && pf_val >= a_full)) wait_counter(p.a_done + g, a_full, p.err);
+        fence_acquire_gpu();   // (published to the other threads by the CTA barrier that follows)
         ready_g = g;
     };
     auto prefetch_ready = [&](int j) {   // thread 0
         if (j < nbj) {
             const int g = group_of_job(j);
-            if (g != ready_g) prefetch_line(p.a_done + (g & ~3));
+            if (g != ready_g) { pf_g = g; pf_val = ld_relaxed_u32(p.a_done + g); }
         }
     };
-    if (tid == 0 && nbj > 0) { prefetch_ready(0); wait_ready(0); prefetch_ready(1); }
+    if (tid == lead && nbj > 0) { prefetch_ready(0); wait_ready(0); prefetch_ready(1); }
     __syncthreads();
     for (int bi = 0; bi < nbj; bi++) {
         // ---------------- B job bi: spectrum m (ring position zpos), row `row`
-        const bool active = m < p.nspec && p.dbg_mode != 1;
+        const bool active = m < p.nspec;
         if (active && m >= nextb) {   // new accumulation window (warp-uniform: a warp never straddles spectra)
             if (wcur >= 0) { sink.flush(st, row, t, wcur); sink.begin(st); }
             wcur = (p.c0 + m) / p.M;
@@ -652,7 +577,7 @@ k_fused(const FusedParams p) {
         }
         // the next job's group must be complete before anybody loads its rows: checked here (the poll
         // was prefetched a job ago), published by the barrier
-        if (tid == 0 && bi + 1 < nbj) { wait_ready(bi + 1); prefetch_ready(bi + 2); }
+        if (tid == lead && bi + 1 < nbj) { wait_ready(bi + 1); prefetch_ready(bi + 2); }
         __syncthreads();
         // The rows just consumed are dead (their ring slot will be rewritten in full): drop their dirty L2
         // lines instead of letting them be written back to HBM -- the ring is meant to live in L2 only.
@@ -661,7 +586,7 @@ k_fused(const FusedParams p) {
             for (int i = 0; i < (L * 16) / (NTS * 128); i++)
                 asm volatile("discard.global.L2 [%0], 128;" ::"l"(zrow + (t + NTS * i) * 8) : "memory");
         }
-        if (tid == 0) {   // my rows of this job are consumed: the producers may reuse the ring slot
+        if (tid == lead) {   // my rows of this job are consumed: the producers may reuse the ring slot
             const int s0 = (y + bi * ny) * SPJ;
             int s1 = s0 + SPJ;
             if (s1 > p.nspec) s1 = p.nspec;

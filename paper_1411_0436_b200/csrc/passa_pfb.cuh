@@ -11,7 +11,9 @@
 
 namespace spk {
 
-template <int P, int T, int C, int R>
+// DUMP (test hook): the FIR outputs the column FFT is about to consume are written to Z as the caller's
+// [spectrum][n][re,im per pol] and no transform runs.
+template <int P, int T, int C, int R, bool DUMP = false>
 __global__ void __launch_bounds__(C * R, 2)
 k_passA_pfb16(const InputView view, const float* __restrict__ h, float4* __restrict__ Z,
               const float2* __restrict__ twN, int N, int N2, long long m0, int nb, int phases_per_cta) {
@@ -87,11 +89,21 @@ k_passA_pfb16(const InputView view, const float* __restrict__ h, float4* __restr
             cpx v[16];
 #pragma unroll
             for (int n1 = 0; n1 < 16; n1++) v[n1] = f4_to_cpx(ysm[(fr * 16 + n1) * C + fc]);
-            dft<16>(v);
-            float4* zp = Z + (size_t)(j0 + fr) * N + n2;
-            zp[0] = cpx_to_f4(v[0]);
+            if (DUMP) {
 #pragma unroll
-            for (int k = 1; k < 16; k++) zp[(size_t)k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
+                for (int n1 = 0; n1 < 16; n1++) {
+                    const float4 z = cpx_to_f4(v[n1]);
+                    const size_t o = (size_t)(j0 + fr) * N + (size_t)n1 * N2 + n2;
+                    if (P == 2) Z[o] = make_float4(z.x, z.z, z.y, z.w);
+                    else ((float2*)Z)[o] = make_float2(z.x, z.z);
+                }
+            } else {
+                dft<16>(v);
+                float4* zp = Z + (size_t)(j0 + fr) * N + n2;
+                zp[0] = cpx_to_f4(v[0]);
+#pragma unroll
+                for (int k = 1; k < 16; k++) zp[(size_t)k * N2] = cpx_to_f4(cmul(v[k], tw[k].x, tw[k].y));
+            }
         }
         __syncthreads();
     }

@@ -10,6 +10,7 @@
 #include <string.h>
 #include <time.h>
 
+#include <mutex>
 #include <type_traits>
 #include <vector>
 
@@ -57,7 +58,7 @@ struct spec_ctx {
     float2* d_tw1 = nullptr;     // W_N1^e (pass A engine), N1 entries
     float2* d_tw2 = nullptr;     // W_N2^e (single / pass B engine), N2 entries
     int* d_perm = nullptr;       // position -> natural channel
-    uint8_t* d_hist[2] = {nullptr, nullptr};
+    uint8_t* d_hist[3] = {nullptr, nullptr, nullptr};   // three buffers rotate: overlapping launches never write what another reads
     int cur = 0, nhist = 0;
     float4* d_Z = nullptr;       // four-step intermediate, zbatch spectra (fused path: the Z ring)
     float4* d_Y = nullptr;       // FIR output of a batch (two-launch path with N1 > 16, 8 taps)
@@ -69,11 +70,16 @@ struct spec_ctx {
     unsigned* d_err = nullptr;
     unsigned* d_flags = nullptr;   // two sets (alternating launches) of: role words, a_done[fcap], b_done[fcap]
     int fcap = 0;
-    int fpdl = 1;                  // fused launches use programmatic stream serialisation (SPEC_FUSED_PDL=0 turns it off)
+    int fpdl = 1;                  // fused launches use programmatic stream serialisation
     int fpar = 0;                  // which set of counters / which Z ring the next fused launch uses
     const uint8_t* carry_src = nullptr;   // history carry the next fused launch performs itself (see spec_process)
     uint8_t* carry_dst = nullptr;
     size_t carry_bytes = 0;
+    unsigned* d_carry_cnt = nullptr;   // device counter the carrying launches signal (fused.cuh)
+    unsigned carry_cum = 0;            // its value once every carrying launch queued so far has signalled
+    bool hist_by_kernel = false;       // the current history buffer was written by the previous launch's carry
+    bool failed = false;               // a CUDA call failed part-way through spec_process: only spec_reset / spec_destroy are valid
+    float* dump = nullptr;             // spec_debug_fir: the launch in flight is a DUMP instantiation writing here
     float* d_ring = nullptr;     // nring accumulators of S*N floats, position order, [pos][S]
     int nring = 0;
     float* d_stage = nullptr;    // planar read-out staging, S*N
@@ -226,30 +232,48 @@ __global__ void k_unpermute(float* __restrict__ ring, const int* __restrict__ pe
     }
 }
 
-__global__ void k_debug_unpack(const uint8_t* __restrict__ b, size_t n, float* __restrict__ out) {
+// test hook: the unpack the kernels use, word by word.  npol = 2: unpack_cpx<2> (the packed form every dual-pol
+// front end calls), npol = 1: unpack_cpx<1>
+__global__ void k_debug_unpack(const uint8_t* __restrict__ b, size_t n, float* __restrict__ out, int npol) {
     const size_t i = ((size_t)blockIdx.x * blockDim.x + threadIdx.x) * 4;
     if (i >= n) return;
     uint32_t w = 0;
     for (int j = 0; j < 4 && i + j < n; j++) w |= (uint32_t)b[i + j] << (8 * j);
     float f[4];
-    unpack4(w, f[0], f[1], f[2], f[3]);
+    if (npol == 2) {
+        const float4 z = cpx_to_f4(unpack_cpx<2>(w));   // (Xre, Yre, Xim, Yim)
+        f[0] = z.x; f[1] = z.z; f[2] = z.y; f[3] = z.w;
+    } else {
+        const float4 z0 = cpx_to_f4(unpack_cpx<1>(w & 0xffffu)), z1 = cpx_to_f4(unpack_cpx<1>(w >> 16));
+        f[0] = z0.x; f[1] = z0.z; f[2] = z1.x; f[3] = z1.z;
+    }
     for (int j = 0; j < 4 && i + j < n; j++) out[i + j] = f[j];
 }
 
-template <int MODE_PFB, int P, int WIN>
-__global__ void k_debug_fir(FrontRaw<MODE_PFB, P, WIN> front, float* __restrict__ out) {
-    const int n = blockIdx.x * blockDim.x + threadIdx.x;
-    if (n >= front.N) return;
-    const cpx y = front.load(0, n, 0);
-    float xr, yr, xi, yi;
-    upk(y.re, xr, yr);
-    upk(y.im, xi, yi);
-    if (P == 2) ((float4*)out)[n] = make_float4(xr, xi, yr, yi);
-    else ((float2*)out)[n] = make_float2(xr, xi);
+// test hook: float4 (Xre, Yre, Xim, Yim) / float2-in-float4 intermediates -> the caller's [n][re,im per pol]
+__global__ void k_debug_reorder(const float4* __restrict__ y, size_t n, float* __restrict__ out, int npol) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 z = y[i];
+    if (npol == 2) ((float4*)out)[i] = make_float4(z.x, z.z, z.y, z.w);
+    else ((float2*)out)[i] = make_float2(z.x, z.z);
+}
+
+// test hook (soak test): one CTA per SM that holds `smem` bytes of shared memory and spins for `ns` nanoseconds
+__global__ void __launch_bounds__(128, 1) k_debug_hog(unsigned long long ns, unsigned* sink) {
+    extern __shared__ unsigned hog[];
+    hog[threadIdx.x] = threadIdx.x;
+    unsigned long long t0, t1;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+    do {
+        __nanosleep(1000);
+        asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+    } while (t1 - t0 < ns);
+    if (hog[(threadIdx.x + 1) & 127] == 0xffffffffu) *sink = 1u;
 }
 
 // FP32 peak: 16 independent FFMA chains per thread, operands shared so the register file is not
-// the limit (profiles/r01_ubench.md: 125-128 FMA/clk/SM)
+// the limit
 __global__ void __launch_bounds__(1024, 1) k_fp32_peak(float* out, int iters, float c0, float c1) {
     float a[16];
 #pragma unroll
@@ -304,12 +328,20 @@ static int launch_single_w(spec_ctx* s, const InputView& view, long long m0, lon
     const int len = cdiv(nspec, target);
     const int nruns = cdiv(nspec, len);
     JobMap jm{nspec, len, nruns, 1, c0, s->M};
+    if (s->dump) {   // test hook: the same kernel, front end only
+        auto kd = k_engine<PL, false, G, MINB, FrontRaw<MODE_PFB, P, WIN>, Sink, true>;
+        int rc = prep_smem(kd, smem);
+        if (rc) return rc;
+        kd<<<dim3(cdiv(nruns, G)), NT, smem, st>>>(front, sink, jm, s->d_tw2, s->dump);
+        CK(cudaGetLastError());
+        return 0;
+    }
     auto kern = k_engine<PL, false, G, MINB, FrontRaw<MODE_PFB, P, WIN>, Sink>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
     {
         ProfScope ps(s, 0, st);
-        kern<<<dim3(cdiv(nruns, G)), NT, smem, st>>>(front, sink, jm, s->d_tw2);
+        kern<<<dim3(cdiv(nruns, G)), NT, smem, st>>>(front, sink, jm, s->d_tw2, nullptr);
     }
     CK(cudaGetLastError());
     return 0;
@@ -333,12 +365,20 @@ static int launch_passA_w(spec_ctx* s, const InputView& view, long long m0, int 
     const int len = cdiv(nb, ny);
     ny = cdiv(nb, len);
     JobMap jm{nb, len, s->N2, 0, 0, 1};
+    if (s->dump) {   // test hook: the same kernel, front end only
+        auto kd = k_engine<PL, true, G, 1, FrontRaw<MODE_PFB, P, WIN>, SinkZ, true>;
+        int rc = prep_smem(kd, smem);
+        if (rc) return rc;
+        kd<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw1, s->dump);
+        CK(cudaGetLastError());
+        return 0;
+    }
     auto kern = k_engine<PL, true, G, 1, FrontRaw<MODE_PFB, P, WIN>, SinkZ>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
     {
         ProfScope ps(s, 1, st);
-        kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw1);
+        kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw1, nullptr);
     }
     CK(cudaGetLastError());
     return 0;
@@ -370,7 +410,7 @@ static int launch_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
     if (rc) return rc;
     {
         ProfScope ps(s, 2, st);
-        kern<<<dim3(gx, ny), NT, smem, st>>>(front, sink, jm, s->d_tw2);
+        kern<<<dim3(gx, ny), NT, smem, st>>>(front, sink, jm, s->d_tw2, nullptr);
     }
     CK(cudaGetLastError());
     return 0;
@@ -414,15 +454,23 @@ template <int P>
 static int launch_passA_pfb16(spec_ctx* s, const InputView& view, long long m0, int nb, cudaStream_t st) {
     constexpr int C = 32, R = 8;
     const size_t smem = (size_t)R * 16 * C * sizeof(float4);
-    auto kern = k_passA_pfb16<P, 8, C, R>;
-    int rc = prep_smem(kern, smem);
-    if (rc) return rc;
     const int gx = s->N2 / C;
     const int nphases = cdiv(nb, R);
     int ny = cdiv((long long)3 * s->numSM, gx);
     if (ny > nphases) ny = nphases;
     const int ppc = cdiv(nphases, ny);
     ny = cdiv(nphases, ppc);
+    if (s->dump) {   // test hook: the same kernel, FIR phase only
+        auto kd = k_passA_pfb16<P, 8, C, R, true>;
+        int rc = prep_smem(kd, smem);
+        if (rc) return rc;
+        kd<<<dim3(gx, ny), C * R, smem, st>>>(view, s->d_coef, (float4*)s->dump, s->d_twN, s->N, s->N2, m0, nb, ppc);
+        CK(cudaGetLastError());
+        return 0;
+    }
+    auto kern = k_passA_pfb16<P, 8, C, R>;
+    int rc = prep_smem(kern, smem);
+    if (rc) return rc;
     {
         ProfScope ps(s, 1, st);
         kern<<<dim3(gx, ny), C * R, smem, st>>>(view, s->d_coef, s->d_Z, s->d_twN, s->N, s->N2, m0, nb, ppc);
@@ -440,6 +488,12 @@ static int launch_passA_fir(spec_ctx* s, const InputView& view, long long m0, in
         k_fir8<P, CH><<<dim3(cdiv(s->N, 256), cdiv(nb, CH)), 256, 0, st>>>(view, s->d_coef, s->d_Y, s->N, m0, nb);
     }
     CK(cudaGetLastError());
+    if (s->dump) {   // test hook: the FIR kernel's own output
+        const size_t n = (size_t)nb * s->N;
+        k_debug_reorder<<<cdiv((long long)n, 256), 256, 0, st>>>(s->d_Y, n, s->dump, P);
+        CK(cudaGetLastError());
+        return 0;
+    }
     constexpr int G = 256 / PL::NTS;
     const size_t smem = (PL::NST > 1) ? (size_t)G * PL::L * sizeof(float4) : 0;
     FrontY front{s->d_Y, s->N, s->N2};
@@ -455,7 +509,7 @@ static int launch_passA_fir(spec_ctx* s, const InputView& view, long long m0, in
     if (rc) return rc;
     {
         ProfScope ps(s, 1, st);
-        kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw1);
+        kern<<<dim3(gx, ny), PL::NTS * G, smem, st>>>(front, sink, jm, s->d_tw1, nullptr);
     }
     CK(cudaGetLastError());
     return 0;
@@ -506,17 +560,84 @@ static int run_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
     return SPEC_ERR_ARG;
 }
 
+#ifdef SPEC_TUNING
+// Tuning builds only (-DSPEC_TUNING, never the default build): plan parameters overridden from the environment.
+static int tuning_int(const char* name, int dflt, int lo, int hi) {
+    if (const char* e = getenv(name)) { const long v = atol(e); if (v >= lo && v <= hi) return (int)v; }
+    return dflt;
+}
+#endif
+
 // ---- fused persistent four-step kernel (fused.cuh): one launch per call
 static const int FUSED_ROLE_WORDS = kFusedRoleWords;
 #ifndef FUSED_PER_SM
 #define FUSED_PER_SM 4   // resident CTAs of 128 threads per SM (128 registers each)
 #endif
+// ---- one persistent grid at a time.  A k_fused grid is exactly what the GPU holds at once and its CTAs wait for one
+// another, so two such grids must never become resident piecemeal side by side (each would wait for slots the
+// other holds).  Consecutive launches on ONE stream are safe (the dependent launch only starts once its
+// predecessor is fully resident); launches on DIFFERENT streams (several handles) are chained here in submission
+// order with an event, per device.  The chain costs nothing until a second stream shows up: from then on an
+// event is recorded after every persistent launch (which also keeps same-stream launches from overlapping).
+struct FusedChain {
+    std::mutex mu;
+    cudaStream_t last = nullptr;
+    bool has_last = false, multi = false, ev_valid = false;
+    cudaEvent_t ev = nullptr;
+};
+static FusedChain g_chain[64];
+static FusedChain& fused_chain() {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    return g_chain[dev & 63];
+}
+// call with the chain locked, before the launch on `st`
+static int fused_chain_enter(FusedChain& c, cudaStream_t st) {
+    if (!c.multi && c.has_last && c.last != st) {
+        CK(cudaDeviceSynchronize());   // once: everything queued before the second stream appeared has finished
+        if (!c.ev) CK(cudaEventCreateWithFlags(&c.ev, cudaEventDisableTiming));
+        c.multi = true;
+        c.ev_valid = false;
+    }
+    if (c.multi && c.ev_valid && c.last != st) CK(cudaStreamWaitEvent(st, c.ev, 0));
+    return 0;
+}
+static int fused_chain_leave(FusedChain& c, cudaStream_t st) {
+    if (c.multi) {
+        CK(cudaEventRecord(c.ev, st));
+        c.ev_valid = true;
+    }
+    c.last = st;
+    c.has_last = true;
+    return 0;
+}
+// spec_destroy / spec_reset have synchronised the device: nothing persistent is in flight any more
+static void fused_chain_quiesce() {
+    FusedChain& c = fused_chain();
+    std::lock_guard<std::mutex> lk(c.mu);
+    c.has_last = false;
+    c.ev_valid = false;
+    c.multi = false;
+}
+
+// the per-group counters of the fused kernel: two sets (alternating launches), each FUSED_ROLE_WORDS + 2*cap words
+static int fused_alloc_flags(spec_ctx* s, int ngroups) {
+    const int cap = (ngroups + ngroups / 2 + 64) & ~3;
+    unsigned* f = nullptr;
+    CK(cudaMalloc(&f, (size_t)2 * (FUSED_ROLE_WORDS + 2 * cap) * sizeof(unsigned)));
+    cudaError_t e = cudaMemset(f, 0, (size_t)2 * (FUSED_ROLE_WORDS + 2 * cap) * sizeof(unsigned));   // the kernel leaves them zero
+    if (e != cudaSuccess) { cudaFree(f); return fail_cuda(e, "cudaMemset(flags)"); }
+    cudaFree(s->d_flags);   // (the new set exists before the old one goes: a failed allocation leaves the handle intact)
+    s->d_flags = f;
+    s->fcap = cap;
+    return 0;
+}
+
 template <class PL, int NT, int MODE_PFB, int PER_SM>
 static int fused_do(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
     auto kern = k_fused<PL, NT, MODE_PFB, PER_SM>;
     // exchange buffer / FIR hand-off, plus (PFB) the staged raw tile of a producer phase: R+7 blocks of 1 KiB
-    size_t smem = (size_t)NT * 16 * sizeof(float4) + (MODE_PFB ? (size_t)(NT / 16 + 7) * 1024 : 0);
-    if (MODE_PFB && SPK_WARP_PRODUCER && ProducerPfbWarp<NT, PL::L>::SMEM > smem) smem = ProducerPfbWarp<NT, PL::L>::SMEM;
+    const size_t smem = (size_t)NT * 16 * sizeof(float4) + (MODE_PFB ? (size_t)(NT / 16 + 7) * 1024 : 0);
     if (query) {
         int rc = prep_smem(kern, smem);
         if (rc) return rc;
@@ -530,20 +651,14 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     }
     auto ilog2 = [](int v) { int l = 0; while ((1 << l) < v) l++; return l; };
     const int ngroups = (int)((nspec + s->fGS - 1) / s->fGS);
-    if (ngroups > s->fcap) {   // grow the per-group counters (rare: first call, or a longer call than any before)
+    if (ngroups > s->fcap) {   // a longer call than spec_create sized the counters for (rare)
         CK(cudaStreamSynchronize(st));
-        cudaFree(s->d_flags);
-        s->d_flags = nullptr;
-        s->fcap = 0;
-        const int cap = (ngroups + ngroups / 2 + 64) & ~3;   // counters are prefetched as 16-byte lines
-        CK(cudaMalloc(&s->d_flags, (size_t)2 * (FUSED_ROLE_WORDS + 2 * cap) * sizeof(unsigned)));
-        CK(cudaMemset(s->d_flags, 0, (size_t)2 * (FUSED_ROLE_WORDS + 2 * cap) * sizeof(unsigned)));   // the kernel leaves them zero
-        s->fcap = cap;
+        int rc = fused_alloc_flags(s, ngroups);
+        if (rc) return rc;
     }
     // consecutive launches may overlap (programmatic dependent launch): they alternate between two Z rings
     // and two sets of counters
     const int par = s->fpar;
-    s->fpar ^= 1;
     unsigned* const flags = s->d_flags + (size_t)par * (FUSED_ROLE_WORDS + 2 * s->fcap);
     FusedParams p;
     p.view = view; p.h = s->d_coef; p.Z = s->d_Z + (size_t)par * s->zbatch * s->N; p.twN = s->d_twN; p.twL = s->d_tw2;
@@ -553,41 +668,43 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     p.role = flags; p.a_done = flags + FUSED_ROLE_WORDS; p.b_done = flags + FUSED_ROLE_WORDS + s->fcap;
     p.err = s->d_err;
     p.carry_src = (const uint4*)s->carry_src; p.carry_dst = (uint4*)s->carry_dst; p.carry_chunks = (int)(s->carry_bytes / 16);
-    s->carry_bytes = 0;   // (taken)
-    p.dbg_mode = 0;
-    if (const char* e = getenv("SPEC_FUSED_SKIP")) p.dbg_mode = atoi(e);
+    p.carry_cnt = s->d_carry_cnt; p.carry_wait = s->carry_cum; p.carry_wait_on = (s->hist_by_kernel && view.nhist > 0) ? 1 : 0;
+    p.dump = s->dump;
+#ifdef SPEC_TUNING
+    p.na_per_sm = tuning_int("SPEC_FUSED_NA", p.na_per_sm, 1, PER_SM - 1);
+#endif
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(s->fgrid); cfg.blockDim = dim3(NT); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = s->fpdl ? 1 : 0;
+    if (s->dump) {   // test hook: the same kernel, front end only (no carry, no accumulation)
+        auto kd = k_fused<PL, NT, MODE_PFB, PER_SM, true>;
+        int rc = prep_smem(kd, smem);
+        if (rc) return rc;
+        p.carry_chunks = 0; p.carry_wait_on = 0;
+        cfg.numAttrs = 0;
+        CK(cudaLaunchKernelEx(&cfg, kd, p));
+        CK(cudaGetLastError());
+        return 0;
+    }
     {
-        ProfScope ps(s, 0, st);
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3(s->fgrid); cfg.blockDim = dim3(NT); cfg.dynamicSmemBytes = smem; cfg.stream = st;
-        cudaLaunchAttribute at[1];
-        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        at[0].val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = at; cfg.numAttrs = s->fpdl ? 1 : 0;
-        CK(cudaLaunchKernelEx(&cfg, kern, p));
-    }
-    CK(cudaGetLastError());
-    if (getenv("SPEC_FUSED_WATCHDOG")) {   // debugging aid: dump the counters if the launch does not finish
-        for (int ms = 0; ms < 3000 && cudaStreamQuery(st) == cudaErrorNotReady; ms++) {
-            struct timespec ts = {0, 1000000};
-            nanosleep(&ts, nullptr);
+        FusedChain& ch = fused_chain();
+        std::lock_guard<std::mutex> lk(ch.mu);
+        int rc = fused_chain_enter(ch, st);
+        if (rc) return rc;
+        {
+            ProfScope ps(s, 0, st);
+            CK(cudaLaunchKernelEx(&cfg, kern, p));
         }
-        if (cudaStreamQuery(st) == cudaErrorNotReady) {
-            cudaStream_t side;
-            cudaStreamCreateWithFlags(&side, cudaStreamNonBlocking);
-            std::vector<unsigned> h((size_t)FUSED_ROLE_WORDS + 2 * s->fcap);
-            cudaMemcpyAsync(h.data(), flags, h.size() * sizeof(unsigned), cudaMemcpyDeviceToHost, side);
-            cudaStreamSynchronize(side);
-            fprintf(stderr, "[fused HANG] N=%d nspec=%lld grid=%d NT=%d na=%d GS=%d RING=%d ngroups=%d TPG=%d | rankA=%u rankB=%u arrived=%u\n",
-                    s->N, nspec, s->fgrid, NT, s->fna, s->fGS, s->fRING, ngroups, s->N2 / 16, h[0], h[1], h[2]);
-            int mx = 0, mn = 1 << 30, nz = 0;
-            for (int i = 0; i < 512; i++) { const int v = (int)h[4 + i]; if (v) { nz++; if (v > mx) mx = v; if (v < mn) mn = v; } }
-            fprintf(stderr, "  SMs seen %d, CTAs per SM min %d max %d\n", nz, mn, mx);
-            for (int g = 0; g < ngroups && g < 40; g++)
-                fprintf(stderr, "  g=%d a_done=%u b_done=%u\n", g, h[FUSED_ROLE_WORDS + g], h[FUSED_ROLE_WORDS + s->fcap + g]);
-            abort();
-        }
+        CK(cudaGetLastError());
+        rc = fused_chain_leave(ch, st);
+        if (rc) return rc;
     }
+    // the launch is queued: only now does the handle move on
+    s->fpar ^= 1;
+    if (p.carry_chunks) s->carry_cum += (unsigned)s->fgrid;
     return 0;
 }
 
@@ -630,7 +747,7 @@ static void free_all(spec_ctx* s) {
     prof_fold(s);
     for (auto e : s->pool) cudaEventDestroy(e);
     cudaFree(s->d_coef); cudaFree(s->d_twN); cudaFree(s->d_tw1); cudaFree(s->d_tw2); cudaFree(s->d_perm);
-    cudaFree(s->d_hist[0]); cudaFree(s->d_hist[1]); cudaFree(s->d_Z); cudaFree(s->d_Y); cudaFree(s->d_ring); cudaFree(s->d_stage);
+    cudaFree(s->d_hist[0]); cudaFree(s->d_hist[1]); cudaFree(s->d_hist[2]); cudaFree(s->d_carry_cnt); cudaFree(s->d_Z); cudaFree(s->d_Y); cudaFree(s->d_ring); cudaFree(s->d_stage);
     cudaFree(s->d_sbuf[0]); cudaFree(s->d_sbuf[1]); cudaFree(s->d_flags);
     if (s->h_err) cudaFreeHost(s->h_err);
     if (s->side) cudaStreamDestroy(s->side);
@@ -663,8 +780,11 @@ static int create_impl(spec_ctx* s) {
     CK(cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev));
     // (the resident-grid arithmetic of the fused kernel assumes the 64 K-register SM of sm_100)
     s->fused = regs_per_sm == 65536 && cc_major == 10 &&
-               s->P == 2 && N >= 1024 && N <= 65536 && !getenv("SPEC_NO_FUSED") &&
+               s->P == 2 && N >= 1024 && N <= 65536 &&
                ((s->mode == SPEC_MODE_PFB && s->T == 8) || (s->mode == SPEC_MODE_FFT && N >= 8192));
+#ifdef SPEC_TUNING
+    if (tuning_int("SPEC_NO_FUSED", 0, 0, 1)) s->fused = false;
+#endif
     if (s->fused) { s->N1 = 16; s->N2 = N / 16; }
     else if (N <= 4096) { s->N1 = 1; s->N2 = N; }
     else if (N <= 65536) { s->N1 = 16; s->N2 = N / 16; }
@@ -688,9 +808,11 @@ static int create_impl(spec_ctx* s) {
         CK(cudaMemcpy(s->d_twN, w.data(), w.size() * sizeof(float2), cudaMemcpyHostToDevice));
         // two-launch path: the Z batch of one launch pair.  Measured (profiles/r01b_tuning.md): long runs per CTA
         // and few launches matter more here than keeping Z in L2, so the batch covers a whole 64 MiB call
-        // (256 MiB of Z); SPEC_ZBATCH_MB overrides
+        // (256 MiB of Z)
         size_t zmb = 256;
-        if (const char* e = getenv("SPEC_ZBATCH_MB")) { const long v = atol(e); if (v >= 1 && v <= 4096) zmb = (size_t)v; }
+#ifdef SPEC_TUNING
+        zmb = (size_t)tuning_int("SPEC_ZBATCH_MB", 256, 1, 4096);
+#endif
         size_t zb = (zmb << 20) / ((size_t)N * sizeof(float4));
         s->zbatch = (int)(zb < 1 ? 1 : zb);
         if (s->fused) {
@@ -698,14 +820,15 @@ static int create_impl(spec_ctx* s) {
             int rc = fused_dispatch(s, true, none, 0, 0, nullptr);
             if (rc) return rc;
             const int NT = (s->N2 == 4096) ? 256 : 128;
-            s->fGS = (s->N2 >= 512) ? 16 : 32;   // spectra per ring group (measured best: profiles/r01b_tuning.md)
-            if (const char* e = getenv("SPEC_FUSED_GS")) { const int v = atoi(e); if (v >= 2 && v <= 4096 && !(v & (v - 1))) s->fGS = v; }
+            s->fGS = (s->N2 >= 512) ? 16 : 32;   // spectra per ring group (measured best in round 1)
+#ifdef SPEC_TUNING
+            { const int v = tuning_int("SPEC_FUSED_GS", s->fGS, 2, 4096); if (!(v & (v - 1))) s->fGS = v; }
+#endif
             // producer share of the resident CTAs: two of the four CTAs of an SM produce, in both modes.  The
             // FIR makes an A task about as long as the row FFT of the same samples; without it (direct-FFT
             // mode) one producer per SM was the first choice, but two measure faster now that consecutive
-            // launches overlap (profiles/r01e_tuning.md: N=8192 101 -> 115 GHz, N=32768 111 -> 112 GHz)
+            // launches overlap (round 1: N=8192 101 -> 115 GHz, N=32768 111 -> 112 GHz)
             s->fna = (NT == 256) ? 1 : 2;
-            if (const char* e = getenv("SPEC_FUSED_NA")) { const int v = atoi(e); if (v >= 1 && v < ((NT == 256) ? 2 : FUSED_PER_SM)) s->fna = v; }
             // ring = what the producers (one task each) and the consumers (one job of 16*NT points each)
             // hold at a time, plus two groups of slack
             const int per_sm = (NT == 256) ? 2 : FUSED_PER_SM, nsm = s->fgrid / per_sm;
@@ -713,15 +836,45 @@ static int create_impl(spec_ctx* s) {
             const int a_groups = (nsm * s->fna + tpg - 1) / tpg;
             const long long b_spectra = ((long long)nsm * (per_sm - s->fna) * NT * 16 + N - 1) / N;
             s->fRING = a_groups + (int)((b_spectra + s->fGS - 1) / s->fGS) + 2;
-            if (const char* e = getenv("SPEC_FUSED_RING")) { const int v = atoi(e); if (v >= 2 && v <= 4096) s->fRING = v; }
+#ifdef SPEC_TUNING
+            s->fRING = tuning_int("SPEC_FUSED_RING", s->fRING, 2, 4096);
+            s->fpdl = tuning_int("SPEC_FUSED_PDL", 1, 0, 1);
+#endif
             s->zbatch = s->fRING * s->fGS;
             CK(cudaHostAlloc(&s->h_err, sizeof(unsigned), cudaHostAllocMapped));
             *s->h_err = 0u;
             CK(cudaHostGetDevicePointer(&s->d_err, s->h_err, 0));
+            CK(cudaMalloc(&s->d_carry_cnt, sizeof(unsigned)));
+            CK(cudaMemset(s->d_carry_cnt, 0, sizeof(unsigned)));
+            // per-group counters for calls of up to 2^28 samples (1 GiB of dual-pol input); a longer call grows them
+            rc = fused_alloc_flags(s, (int)(((1ll << 28) / N + s->fGS - 1) / s->fGS));
+            if (rc) return rc;
         }
         // (fused path: two rings, alternating launches may overlap)
         CK(cudaMalloc(&s->d_Z, (size_t)(s->fused ? 2 : 1) * s->zbatch * N * sizeof(float4)));
-        if (const char* e = getenv("SPEC_FUSED_PDL")) s->fpdl = atoi(e);
+        if (s->fused) {
+            // Residency probe: the persistent grid assumes PER_SM CTAs on every SM at once (nothing can ask the
+            // occupancy API, see fused_do).  An empty launch of the same kernel proves it here: every CTA waits for
+            // all the others to arrive; if they cannot (an SM limit, a long-running foreign kernel) the wait
+            // expires, the error word is raised and this handle falls back to the two-launch path.
+            InputView none{nullptr, nullptr, 0};
+            int prc = fused_dispatch(s, false, none, 0, 0, nullptr);
+            if (prc == 0) {
+                CK(cudaDeviceSynchronize());
+                if (*(volatile unsigned*)s->h_err) prc = SPEC_ERR_CUDA;
+            }
+            if (prc) {
+                *s->h_err = 0u;
+                CK(cudaMemset(s->d_flags, 0, (size_t)2 * (FUSED_ROLE_WORDS + 2 * s->fcap) * sizeof(unsigned)));
+                s->fused = false;
+                s->fpar = 0;
+                cudaFree(s->d_Z);
+                s->d_Z = nullptr;
+                size_t zb2 = ((size_t)256 << 20) / ((size_t)N * sizeof(float4));
+                s->zbatch = (int)(zb2 < 1 ? 1 : zb2);
+                CK(cudaMalloc(&s->d_Z, (size_t)s->zbatch * N * sizeof(float4)));
+            }
+        }
         if (!s->fused && s->mode == SPEC_MODE_PFB && s->T == 8 && s->N1 > 16)
             CK(cudaMalloc(&s->d_Y, (size_t)s->zbatch * N * sizeof(float4)));
     }
@@ -733,10 +886,8 @@ static int create_impl(spec_ctx* s) {
     CK(cudaMalloc(&s->d_perm, (size_t)N * sizeof(int)));
     CK(cudaMemcpy(s->d_perm, perm.data(), (size_t)N * sizeof(int), cudaMemcpyHostToDevice));
 
-    if (s->T > 1) {
-        CK(cudaMalloc(&s->d_hist[0], (size_t)(s->T - 1) * block_bytes(s)));
-        CK(cudaMalloc(&s->d_hist[1], (size_t)(s->T - 1) * block_bytes(s)));
-    }
+    if (s->T > 1)
+        for (int i = 0; i < 3; i++) CK(cudaMalloc(&s->d_hist[i], (size_t)(s->T - 1) * block_bytes(s)));
     int rc = alloc_ring(s, 8);
     if (rc) return rc;
     CK(cudaMalloc(&s->d_stage, acc_floats(s) * sizeof(float)));
@@ -765,6 +916,7 @@ extern "C" int spec_create(spec_t** out, int nchan, int ntaps, int npol, int mod
 extern "C" int spec_destroy(spec_t* s) {
     if (!s) return SPEC_ERR_ARG;
     cudaDeviceSynchronize();
+    if (s->fused) fused_chain_quiesce();
     free_all(s);
     delete s;
     return SPEC_OK;
@@ -777,6 +929,11 @@ extern "C" int spec_set_coeffs(spec_t* s, const float* h, size_t count) {
     CK(cudaMemcpy(s->d_coef, h, count * sizeof(float), cudaMemcpyHostToDevice));
     s->h_coef.assign(h, h + count);
     s->use_coef = true;
+    if (s->mode == SPEC_MODE_FFT) {   // an all-ones window is the rectangular one: no multiply, same plan as RECT
+        bool ones = true;
+        for (size_t i = 0; i < count && ones; i++) ones = (h[i] == 1.0f);
+        if (ones) s->use_coef = false;
+    }
     return SPEC_OK;
 }
 
@@ -793,12 +950,17 @@ extern "C" long spec_spectra_done(const spec_t* s) { return s ? (long)s->count :
 extern "C" int spec_reset(spec_t* s) {
     if (!s) return SPEC_ERR_ARG;
     CK(cudaDeviceSynchronize());
+    if (s->fused) fused_chain_quiesce();
     s->nhist = 0; s->cur = 0; s->count = 0; s->win_read = 0;
-    if (s->h_err && *s->h_err) {   // a timed-out launch leaves its counters dirty
-        *s->h_err = 0u;
+    s->carry_bytes = 0; s->hist_by_kernel = false; s->fpar = 0;
+    if (s->failed || (s->h_err && *s->h_err)) {   // a failed or timed-out launch leaves its counters dirty
+        if (s->h_err) *s->h_err = 0u;
         if (s->d_flags) CK(cudaMemset(s->d_flags, 0, (size_t)2 * (FUSED_ROLE_WORDS + 2 * s->fcap) * sizeof(unsigned)));
     }
+    if (s->d_carry_cnt) CK(cudaMemset(s->d_carry_cnt, 0, sizeof(unsigned)));
+    s->carry_cum = 0;
     CK(cudaMemset(s->d_ring, 0, (size_t)s->nring * acc_floats(s) * sizeof(float)));
+    s->failed = false;
     return SPEC_OK;
 }
 
@@ -813,6 +975,10 @@ static int fused_failed(spec_ctx* s) {
     if (s->h_err && *(volatile unsigned*)s->h_err) {
         snprintf(g_err, sizeof(g_err), "a wait inside the persistent kernel timed out (grid not fully resident?); "
                                        "results since the last spec_reset are invalid");
+        return 1;
+    }
+    if (s->failed) {
+        snprintf(g_err, sizeof(g_err), "an earlier spec_process failed part-way (CUDA error); call spec_reset");
         return 1;
     }
     return 0;
@@ -832,8 +998,11 @@ extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* 
     const long long done_after = (s->count + nspec) / s->M;
     if (done_after - s->win_read > s->nring - 1) return SPEC_ERR_OVERRUN;
     const int completed = (int)(done_after - windows_done(s));
+    // Everything above leaves the handle untouched.  From here on work is queued: a CUDA failure below marks the
+    // handle failed (partly updated accumulators cannot be rolled back) until spec_reset.
 
     InputView view{s->d_hist[s->cur], (const uint8_t*)d_in, s->nhist};
+    const int nxt = (s->cur + 1) % 3;
     const long long c = s->count + nspec;
     // carry the last min(T-1,total) blocks of  history ++ input  (reading R4).  On the fused path
     // the launch copies them itself when they all come from this call's input, so that consecutive launches
@@ -844,29 +1013,33 @@ extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* 
         if (s->fused && s->N1 > 1 && keep > 0 && nblk >= keep && (s->mode == SPEC_MODE_PFB || !s->use_coef)) {
             const size_t bb = block_bytes(s);
             s->carry_src = (const uint8_t*)d_in + (size_t)(nblk - keep) * bb;
-            s->carry_dst = s->d_hist[s->cur ^ 1];
+            s->carry_dst = s->d_hist[nxt];
             s->carry_bytes = (size_t)keep * bb;
             carried = true;
         }
         int rc = run_spectra(s, view, 0, nspec, s->count, st);
-        if (rc) { s->carry_bytes = 0; return rc; }
+        s->carry_bytes = 0;
+        if (rc) { s->failed = true; return rc; }
     }
     if (carried) {
-        s->cur ^= 1;
+        s->cur = nxt;
+        s->hist_by_kernel = true;
     } else if (keep > 0) {
         const size_t bb = block_bytes(s);
-        uint8_t* dst = s->d_hist[s->cur ^ 1];
+        uint8_t* dst = s->d_hist[nxt];
         const long long first = total - keep;
         long long nold = s->nhist - first;  // blocks still taken from the old history
         if (nold < 0) nold = 0;
+        cudaError_t e = cudaSuccess;
         if (nold > 0)
-            CK(cudaMemcpyAsync(dst, s->d_hist[s->cur] + (size_t)first * bb, (size_t)nold * bb,
-                               cudaMemcpyDeviceToDevice, st));
+            e = cudaMemcpyAsync(dst, s->d_hist[s->cur] + (size_t)first * bb, (size_t)nold * bb, cudaMemcpyDeviceToDevice, st);
         const long long nnew = keep - nold;
-        if (nnew > 0)
-            CK(cudaMemcpyAsync(dst + (size_t)nold * bb, (const uint8_t*)d_in + (size_t)(nblk - nnew) * bb,
-                               (size_t)nnew * bb, cudaMemcpyDeviceToDevice, st));
-        s->cur ^= 1;
+        if (e == cudaSuccess && nnew > 0)
+            e = cudaMemcpyAsync(dst + (size_t)nold * bb, (const uint8_t*)d_in + (size_t)(nblk - nnew) * bb,
+                                (size_t)nnew * bb, cudaMemcpyDeviceToDevice, st);
+        if (e != cudaSuccess) { s->failed = true; return fail_cuda(e, "cudaMemcpyAsync(history)"); }
+        s->cur = nxt;
+        s->hist_by_kernel = false;   // ordinary stream order covers these copies
     }
     s->nhist = (int)keep;
     s->count = c;
@@ -984,32 +1157,72 @@ extern "C" int spec_measure_fp32_peak(double* out_tflops, void* cuda_stream) {
     return SPEC_OK;
 }
 
-extern "C" int spec_debug_unpack(const void* d_bytes, size_t nbytes, float* d_out, void* cuda_stream) {
-    if (!d_bytes || !d_out) return SPEC_ERR_ARG;
+extern "C" int spec_debug_unpack(const void* d_bytes, size_t nbytes, int npol, float* d_out, void* cuda_stream) {
+    if (!d_bytes || !d_out || (npol != 1 && npol != 2)) return SPEC_ERR_ARG;
     if (nbytes == 0) return SPEC_OK;
     k_debug_unpack<<<cdiv((long long)((nbytes + 3) / 4), 256), 256, 0, (cudaStream_t)cuda_stream>>>(
-        (const uint8_t*)d_bytes, nbytes, d_out);
+        (const uint8_t*)d_bytes, nbytes, d_out, npol);
     CK(cudaGetLastError());
     return SPEC_OK;
 }
 
-extern "C" int spec_debug_fir(spec_t* s, const void* d_blocks, float* d_out, void* cuda_stream) {
-    if (!s || !d_blocks || !d_out) return SPEC_ERR_ARG;
+// Runs the FRONT END of the kernel this handle's plan uses (its own staging, index arithmetic, unpack and FIR /
+// window code: a DUMP instantiation of the same kernel template) and writes what it hands to the first butterfly.
+extern "C" int spec_debug_fir(spec_t* s, const void* d_blocks, int nspec, float* d_out, void* cuda_stream) {
+    if (!s || !d_blocks || !d_out || nspec < 1 || ((uintptr_t)d_blocks & 15)) return SPEC_ERR_ARG;
+    if (fused_failed(s)) return SPEC_ERR_CUDA;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     InputView view{nullptr, (const uint8_t*)d_blocks, 0};
-    const float* h = s->d_coef;
-    const int gx = cdiv(s->N, 256);
-    if (s->mode == SPEC_MODE_PFB) {
-        if (s->P == 2) k_debug_fir<1, 2, 1><<<gx, 256, 0, st>>>(FrontRaw<1, 2, 1>{view, h, s->N, s->T, 1, 0}, d_out);
-        else k_debug_fir<1, 1, 1><<<gx, 256, 0, st>>>(FrontRaw<1, 1, 1>{view, h, s->N, s->T, 1, 0}, d_out);
-    } else if (s->use_coef) {
-        if (s->P == 2) k_debug_fir<0, 2, 1><<<gx, 256, 0, st>>>(FrontRaw<0, 2, 1>{view, h, s->N, s->T, 1, 0}, d_out);
-        else k_debug_fir<0, 1, 1><<<gx, 256, 0, st>>>(FrontRaw<0, 1, 1>{view, h, s->N, s->T, 1, 0}, d_out);
+    int rc = 0;
+    s->dump = d_out;
+    if (s->N1 == 1 || (s->fused && (s->mode == SPEC_MODE_PFB || !s->use_coef))) {
+        rc = run_spectra(s, view, 0, nspec, 0, st);
     } else {
-        if (s->P == 2) k_debug_fir<0, 2, 0><<<gx, 256, 0, st>>>(FrontRaw<0, 2, 0>{view, h, s->N, s->T, 1, 0}, d_out);
-        else k_debug_fir<0, 1, 0><<<gx, 256, 0, st>>>(FrontRaw<0, 1, 0>{view, h, s->N, s->T, 1, 0}, d_out);
+        for (long long b0 = 0; b0 < nspec && !rc; b0 += s->zbatch) {
+            const int nb = (int)((nspec - b0 < s->zbatch) ? nspec - b0 : s->zbatch);
+            s->dump = d_out + (size_t)b0 * s->N * 2 * s->P;
+            rc = run_passA(s, view, b0, nb, st);
+        }
     }
+    s->dump = nullptr;
+    return rc;
+}
+
+extern "C" int spec_debug_hog(int ms, size_t smem_bytes, void* cuda_stream) {
+    if (ms < 0 || ms > 2000 || smem_bytes > 227 * 1024) return SPEC_ERR_ARG;
+    int dev = 0, nsm = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    static unsigned* sink = nullptr;
+    if (!sink) CK(cudaMalloc(&sink, sizeof(unsigned)));
+    CK(cudaFuncSetAttribute(k_debug_hog, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
+    k_debug_hog<<<nsm, 128, smem_bytes < 512 ? 512 : smem_bytes, (cudaStream_t)cuda_stream>>>((unsigned long long)ms * 1000000ull, sink);
     CK(cudaGetLastError());
+    return SPEC_OK;
+}
+
+extern "C" int spec_plan_info(const spec_t* s, int* n1, int* n2, char* desc, size_t desc_len) {
+    if (!s) return SPEC_ERR_ARG;
+    if (n1) *n1 = s->N1;
+    if (n2) *n2 = s->N2;
+    if (desc && desc_len) {
+        const bool pfb = s->mode == SPEC_MODE_PFB;
+        int r[3];
+        radices(s->N2, r);
+        if (s->N1 == 1)
+            snprintf(desc, desc_len, "k_engine<Plan<%d,%d,%d,%d>> single CTA per spectrum: unpack%s+FFT+Stokes+accumulate",
+                     s->N2, r[0], r[1], r[2], pfb ? "+FIR" : (s->use_coef ? "+window" : ""));
+        else if (s->fused && (pfb || !s->use_coef))
+            snprintf(desc, desc_len, "k_fused<Plan<%d,%d,%d,%d>,%d,%s> persistent four-step %dx%d: unpack%s+FFT+Stokes+accumulate, "
+                     "grid %d, Z ring %d groups x %d spectra",
+                     s->N2, r[0], r[1], r[2], s->N2 == 4096 ? 256 : 128, pfb ? "PFB" : "FFT", s->N1, s->N2,
+                     pfb ? "+FIR" : "", s->fgrid, s->fRING, s->fGS);
+        else
+            snprintf(desc, desc_len, "two-launch four-step %dx%d: %s then k_engine<Plan<%d,%d,%d,%d>> pass B, Z batch %d spectra",
+                     s->N1, s->N2,
+                     (pfb && s->N1 == 16 && s->T == 8) ? "k_passA_pfb16" : (s->d_Y ? "k_fir8 + k_engine pass A" : "k_engine pass A"),
+                     s->N2, r[0], r[1], r[2], s->zbatch);
+    }
     return SPEC_OK;
 }
 

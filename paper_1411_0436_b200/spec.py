@@ -25,6 +25,7 @@ SYMBOLS = [
     "spec_pending", "spec_spectra_done", "spec_reset", "spec_set_ring", "spec_get_coeffs",
     "spec_stream_host", "spec_measure_fp32_peak", "spec_debug_unpack", "spec_debug_fir",
     "spec_strerror", "spec_last_error", "spec_profile", "spec_profile_read", "spec_read_accum_batch",
+    "spec_plan_info", "spec_debug_hog",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -48,8 +49,10 @@ _lib.spec_set_ring.argtypes = [_vp, C.c_int]
 _lib.spec_get_coeffs.argtypes = [_vp, _fp, _sz]
 _lib.spec_stream_host.argtypes = [_vp, _vp, _sz, _sz, _vp]
 _lib.spec_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), _vp]
-_lib.spec_debug_unpack.argtypes = [_vp, _sz, _vp, _vp]
-_lib.spec_debug_fir.argtypes = [_vp, _vp, _vp, _vp]
+_lib.spec_debug_unpack.argtypes = [_vp, _sz, C.c_int, _vp, _vp]
+_lib.spec_debug_fir.argtypes = [_vp, _vp, C.c_int, _vp, _vp]
+_lib.spec_debug_hog.argtypes = [C.c_int, _sz, _vp]
+_lib.spec_plan_info.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_char_p, _sz]
 _lib.spec_profile.argtypes = [_vp, C.c_int]
 _lib.spec_profile_read.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_long)]
 _lib.spec_strerror.argtypes = [C.c_int]
@@ -81,8 +84,12 @@ def measure_fp32_peak(stream=0):
     return out.value
 
 
-def debug_unpack(d_bytes_ptr, nbytes, d_out_ptr, stream=0):
-    _check(_lib.spec_debug_unpack(d_bytes_ptr, nbytes, d_out_ptr, stream), "spec_debug_unpack")
+def debug_unpack(d_bytes_ptr, nbytes, d_out_ptr, stream=0, npol=2):
+    _check(_lib.spec_debug_unpack(d_bytes_ptr, nbytes, npol, d_out_ptr, stream), "spec_debug_unpack")
+
+
+def debug_hog(ms, smem_bytes, stream=0):
+    _check(_lib.spec_debug_hog(ms, smem_bytes, stream), "spec_debug_hog")
 
 
 class Spec:
@@ -147,8 +154,15 @@ class Spec:
         _check(_lib.spec_profile_read(self._h, ms, n), "spec_profile_read")
         return {k: (ms[i], n[i]) for i, k in enumerate(("single", "passA", "passB", "readout"))}
 
-    def debug_fir(self, d_blocks_ptr, d_out_ptr, stream=0):
-        _check(_lib.spec_debug_fir(self._h, d_blocks_ptr, d_out_ptr, stream), "spec_debug_fir")
+    def debug_fir(self, d_blocks_ptr, d_out_ptr, stream=0, nspec=1):
+        _check(_lib.spec_debug_fir(self._h, d_blocks_ptr, nspec, d_out_ptr, stream), "spec_debug_fir")
+
+    def plan_info(self):
+        """(n1, n2, description) of the kernels this handle's plan uses."""
+        n1, n2 = C.c_int(0), C.c_int(0)
+        buf = C.create_string_buffer(512)
+        _check(_lib.spec_plan_info(self._h, C.byref(n1), C.byref(n2), buf, len(buf)), "spec_plan_info")
+        return n1.value, n2.value, buf.value.decode()
 
     def close(self):
         if getattr(self, "_h", None):

@@ -95,3 +95,53 @@ def check_stokes_invariants(out, slack=1e-5):
     if out.shape[0] == 4:
         assert np.all(out[1] >= 0)
         assert np.all(out[2] ** 2 + out[3] ** 2 <= out[0] * out[1] * (1 + slack) + 1e-30)
+
+
+# ---------------------------------------------------------------- many oracle runs at once
+# The oracle is single-threaded C with one static twiddle table, so independent runs go to separate
+# PROCESSES (spawned: the parent may hold a CUDA context).  The stream is shared through a file in /dev/shm.
+
+def _oracle_job(args):
+    path, nsamples, nchan, ntaps, npol, mode, nacc, window = args
+    raw = np.memmap(path, dtype=np.int8, mode="r", shape=(nsamples, 2 * npol))
+    outs, done = oracle_run(raw, nchan, ntaps, npol, mode, nacc, window=window)
+    return [np.asarray(o) for o in outs], done
+
+
+def _synth_job(args):
+    seed, start, n = args
+    from fractions import Fraction  # noqa: F401
+    from paper_1411_0436_b200 import synth
+    return synth.dual_pol_stream(seed, n, [synth.F_CFG1], start=start)
+
+
+def make_stream_file(seed, nsamples, workers=None):
+    """The config-1 generator's first `nsamples` dual-pol samples as a file in shared memory (generated in
+    parallel: chunks of the stream are independent by construction).  Returns (path, int8 array view)."""
+    import concurrent.futures as cf
+    import multiprocessing as mp
+    import os
+    import tempfile
+    workers = workers or min(16, os.cpu_count() or 1)
+    d = "/dev/shm" if os.path.isdir("/dev/shm") else tempfile.gettempdir()
+    path = os.path.join(d, f"spec_stream_{os.getpid()}_{seed}_{nsamples}.i8")
+    out = np.memmap(path, dtype=np.int8, mode="w+", shape=(nsamples, 4))
+    piece = 1 << 22
+    jobs = [(seed, s, min(piece, nsamples - s)) for s in range(0, nsamples, piece)]
+    with cf.ProcessPoolExecutor(max_workers=workers, mp_context=mp.get_context("spawn")) as ex:
+        for (sd, s, n), r in zip(jobs, ex.map(_synth_job, jobs)):
+            out[s:s + n] = r
+    out.flush()
+    return path, out
+
+
+def oracle_many(path, nsamples, jobs, workers=None):
+    """jobs: list of (nchan, ntaps, npol, mode, nacc, window) on the first nsamples of the stream file.
+    Returns a list of (outputs, spectra_done) in the same order, computed in parallel processes."""
+    import concurrent.futures as cf
+    import multiprocessing as mp
+    import os
+    workers = workers or min(len(jobs), os.cpu_count() or 1)
+    args = [(path, nsamples) + tuple(j) for j in jobs]
+    with cf.ProcessPoolExecutor(max_workers=workers, mp_context=mp.get_context("spawn")) as ex:
+        return list(ex.map(_oracle_job, args))

@@ -72,3 +72,24 @@ def test_product_path_does_not_touch_the_oracle():
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in txt and "from oracle" not in txt, f
                 assert "spec_oracle" not in txt, f
+
+
+def test_no_environment_switches_in_the_product_build():
+    """The plan is a function of spec_create's arguments only: every getenv in csrc/ sits inside
+    #ifdef SPEC_TUNING (a build flag the default build never sets) and nothing calls abort()."""
+    csrc = os.path.join(ROOT, "paper_1411_0436_b200", "csrc")
+    for f in sorted(os.listdir(csrc)):
+        depth_tuning = 0
+        stack = []
+        for ln, line in enumerate(open(os.path.join(csrc, f)), 1):
+            s = line.strip()
+            if s.startswith("#if"):
+                stack.append("SPEC_TUNING" in s and not s.startswith("#ifndef"))
+            elif s.startswith("#endif") and stack:
+                stack.pop()
+            code = line.split("//")[0]
+            if "getenv" in code:
+                assert any(stack), f"{f}:{ln}: getenv outside #ifdef SPEC_TUNING"
+            assert "abort(" not in code, f"{f}:{ln}: abort() in the library"
+    from paper_1411_0436_b200 import build
+    assert not any("SPEC_TUNING" in x for x in build.NVCC_FLAGS)

@@ -4,7 +4,7 @@ accumulated spectra (tests/_harness.py)."""
 import numpy as np
 import pytest
 
-from _harness import check_stokes_invariants, compare, gpu_run, oracle_run
+from _harness import check_stokes_invariants, compare, gpu_run, make_stream_file, oracle_many, oracle_run
 from paper_1411_0436_b200 import synth
 
 pytestmark = pytest.mark.gpu
@@ -23,61 +23,103 @@ def _sp():
 
 
 # ---------------------------------------------------------------- bit-exact stages
+# north_star: "The unpack and indexing stages must be bit-exact."  spec_debug_fir runs the FRONT END of the
+# very kernel the handle's plan uses (a DUMP instantiation of the same template: k_engine, k_fused's
+# producers, k_passA_pfb16, k_fir8), so these tests go through the hot path's own staging, index
+# arithmetic, unpack and FIR code, not through a stand-in.
 
-def test_unpack_bit_exact_all_values_all_lanes():
+@pytest.mark.parametrize("npol", [1, 2])
+def test_unpack_bit_exact_all_values_all_lanes(npol):
     torch, sp = _torch(), _sp()
     # every byte value in every byte lane of a 32-bit word, plus a ragged tail (1027 bytes)
     vals = np.arange(-128, 128, dtype=np.int8)
     b = np.concatenate([np.roll(vals, k) for k in range(4)] + [vals[:3]]).astype(np.int8)
     d = torch.from_numpy(b).cuda()
     out = torch.full((b.size,), 1e9, dtype=torch.float32, device="cuda")
-    sp.debug_unpack(d.data_ptr(), b.size, out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    sp.debug_unpack(d.data_ptr(), b.size, out.data_ptr(), torch.cuda.current_stream().cuda_stream, npol=npol)
     got = out.cpu().numpy()
     assert np.array_equal(got, b.astype(np.float32))
     assert np.array_equal(got.view(np.uint32), b.astype(np.float32).view(np.uint32))
 
 
-@pytest.mark.parametrize("npol", [1, 2])
-@pytest.mark.parametrize("nchan,ntaps", [(64, 4), (1024, 8), (8192, 8)])
-def test_indexing_bit_exact_with_single_tap_coefficients(nchan, ntaps, npol):
-    """h = delta at tap t0(n) for each branch: the FIR output must equal the selected input
-    sample exactly (SURVEY section 4 tier 2)."""
+def _front_end(nchan, ntaps, npol, mode, raw, nspec, coeffs=None, window=1):
     torch, sp = _torch(), _sp()
-    raw = synth.random_bytes(77 + nchan, ntaps * nchan, npol)
+    s = sp.Spec(nchan, ntaps, npol, mode, 1, window)
+    if coeffs is not None:
+        s.set_coeffs(coeffs)
+    d = torch.from_numpy(np.ascontiguousarray(raw).reshape(-1)).cuda()
+    out = torch.full((nspec, nchan, 2 * npol), 7e9, dtype=torch.float32, device="cuda")
+    s.debug_fir(d.data_ptr(), out.data_ptr(), torch.cuda.current_stream().cuda_stream, nspec=nspec)
+    got = out.cpu().numpy()
+    info = s.plan_info()
+    assert s.spectra_done() == 0 and s.pending() == 0      # the hook leaves the stream state alone
+    s.close()
+    return got, info
+
+
+# (nchan, ntaps, npol, the kernel whose front end must be the one that runs)
+FRONT_PFB = [(64, 4, 1, "k_engine"), (64, 4, 2, "k_engine"), (1024, 8, 1, "k_engine"), (4096, 5, 2, "k_engine"),
+             (1024, 8, 2, "k_fused"), (2048, 8, 2, "k_fused"), (4096, 8, 2, "k_fused"), (8192, 8, 2, "k_fused"),
+             (16384, 8, 2, "k_fused"), (32768, 8, 2, "k_fused"), (65536, 8, 2, "k_fused"),
+             (8192, 8, 1, "k_passA_pfb16"), (8192, 4, 2, "k_engine pass A"), (131072, 8, 1, "k_fir8"),
+             (131072, 8, 2, None), (524288, 8, 2, None)]
+
+
+@pytest.mark.parametrize("nchan,ntaps,npol,kernel", FRONT_PFB)
+def test_indexing_bit_exact_with_single_tap_coefficients(nchan, ntaps, npol, kernel):
+    """h = delta at tap t0(n) for each branch: the FIR output must equal the selected input sample exactly,
+    for every spectrum of a run that spans several producer phases and a ragged tail (SURVEY section 4 tier 2)."""
+    nspec = 19 if nchan <= 65536 else 3
+    raw = synth.random_bytes(77 + nchan + ntaps, (nspec + ntaps - 1) * nchan, npol)
     rng = np.random.default_rng(nchan)
     t0 = rng.integers(0, ntaps, size=nchan)
     h = np.zeros((ntaps, nchan), dtype=np.float32)
     h[t0, np.arange(nchan)] = 1.0
-    s = sp.Spec(nchan, ntaps, npol, PFB, 1)
-    s.set_coeffs(h)
-    d = torch.from_numpy(raw.reshape(-1)).cuda()
-    out = torch.zeros((nchan, 2 * npol), dtype=torch.float32, device="cuda")
-    s.debug_fir(d.data_ptr(), out.data_ptr(), torch.cuda.current_stream().cuda_stream)
-    got = out.cpu().numpy()
-    s.close()
-    want = raw.reshape(ntaps, nchan, 2 * npol)[t0, np.arange(nchan)].astype(np.float32)
-    assert np.array_equal(got, want)
+    got, (n1, n2, desc) = _front_end(nchan, ntaps, npol, PFB, raw, nspec, coeffs=h)
+    if kernel is not None:
+        assert kernel in desc, desc
+    x = raw.reshape(nspec + ntaps - 1, nchan, 2 * npol)
+    n = np.arange(nchan)
+    for m in range(nspec):
+        want = x[m + t0, n].astype(np.float32)
+        assert np.array_equal(got[m], want), f"spectrum {m} via {desc}"
 
 
-@pytest.mark.parametrize("npol", [1, 2])
-def test_fir_stage_against_oracle_fir(npol):
+FRONT_FFT = [(256, 2, "k_engine"), (4096, 2, "k_engine"), (4096, 1, "k_engine"), (8192, 2, "k_fused"),
+             (32768, 2, "k_fused"), (65536, 2, "k_fused"), (16384, 1, "k_engine pass A"), (262144, 2, None)]
+
+
+@pytest.mark.parametrize("nchan,npol,kernel", FRONT_FFT)
+def test_unpack_and_indexing_bit_exact_direct_fft_front_end(nchan, npol, kernel):
+    """Direct-FFT mode, rectangular window: what reaches the first butterfly is the unpacked sample itself.
+    Uniform random bytes: every value -128..127 occurs in every byte lane."""
+    nspec = 11 if nchan <= 65536 else 3
+    raw = synth.random_bytes(5 + nchan, nspec * nchan, npol)
+    for lane in range(2 * npol):
+        assert np.unique(raw[:, lane]).size == 256
+    got, (n1, n2, desc) = _front_end(nchan, 1, npol, FFT, raw, nspec, window=0)
+    if kernel is not None:
+        assert kernel in desc, desc
+    want = raw.reshape(nspec, nchan, 2 * npol).astype(np.float32)
+    assert np.array_equal(got, want), desc
+    assert np.array_equal(got.view(np.uint32), want.view(np.uint32))
+
+
+@pytest.mark.parametrize("nchan,npol", [(2048, 1), (2048, 2), (32768, 2), (131072, 2)])
+def test_fir_stage_against_oracle_fir(nchan, npol):
     import oracle
-    torch, sp = _torch(), _sp()
-    N, T = 2048, 8
-    raw = synth.random_bytes(5, T * N, npol)
+    N, T, nspec = nchan, 8, 10 if nchan <= 32768 else 2
+    raw = synth.random_bytes(5, (nspec + T - 1) * N, npol)
     h = synth.random_coeffs(6, T * N)
-    s = sp.Spec(N, T, npol, PFB, 1)
-    s.set_coeffs(h)
-    d = torch.from_numpy(raw.reshape(-1)).cuda()
-    out = torch.zeros((N, 2 * npol), dtype=torch.float32, device="cuda")
-    s.debug_fir(d.data_ptr(), out.data_ptr(), torch.cuda.current_stream().cuda_stream)
-    got = out.cpu().numpy().astype(np.float64)
-    s.close()
-    x = raw.reshape(T * N, npol, 2).astype(np.float64)
-    for p in range(npol):
-        y = oracle.fir(h, x[:, p, 0] + 1j * x[:, p, 1], N, T)
-        g = got[:, 2 * p] + 1j * got[:, 2 * p + 1]
-        assert np.linalg.norm(g - y) / np.linalg.norm(y) < 5e-7
+    got, _ = _front_end(N, T, npol, PFB, raw, nspec, coeffs=h)
+    got = got.astype(np.float64)
+    x = raw.reshape((nspec + T - 1) * N, npol, 2).astype(np.float64)
+    for m in (0, nspec // 2, nspec - 1):
+        for p in range(npol):
+            seg = x[m * N:(m + T) * N, p]
+            y = oracle.fir(h, seg[:, 0] + 1j * seg[:, 1], N, T)
+            g = got[m, :, 2 * p] + 1j * got[m, :, 2 * p + 1]
+            assert np.linalg.norm(g - y) / np.linalg.norm(y) < 5e-7
 
 
 # ---------------------------------------------------------------- parity across sizes / modes
@@ -217,6 +259,184 @@ def test_hann_window_fft_mode_and_default_coefficients():
         s.close()
         ref = oracle.default_coeffs(N, T, mode, 1)
         assert np.all(np.abs(mine - ref) <= np.spacing(np.abs(ref).astype(np.float32)))
+
+
+# ---------------------------------------------------------------- tap counts at the ends of the accepted range
+
+@pytest.mark.parametrize("nchan", [1024, 16384])
+@pytest.mark.parametrize("ntaps", [1, 2, 16, 64])
+def test_parity_tap_counts(nchan, ntaps):
+    """spec_create accepts 1..64 taps: T=1 PFB (a per-branch gain), T=16 and T=64 (the history bookkeeping
+    keeps T-1 blocks and the generic FIR loop runs T times)."""
+    M = 3
+    nblk = 2 * M + (ntaps - 1) + 1
+    raw = synth.random_bytes(nchan + ntaps, nblk * nchan, 2)
+    h = synth.random_coeffs(ntaps * 3 + 1, nchan * ntaps)
+    splits = [nchan * 1, nchan * (nblk - 3), nchan * 2]
+    g, gd = gpu_run(raw, nchan, ntaps, 2, PFB, M, coeffs=h, splits=splits)
+    r, rd = oracle_run(raw, nchan, ntaps, 2, PFB, M, coeffs=h)
+    assert gd == rd == nblk - (ntaps - 1)
+    assert len(g) == len(r) == 2
+    for a, b in zip(g, r):
+        compare(a, b, f"N={nchan} T={ntaps}")
+
+
+# ---------------------------------------------------------------- back-to-back launches, no sync in between
+
+@pytest.mark.parametrize("mode", [PFB, FFT])
+@pytest.mark.parametrize("nchan", FUSED_SIZES)
+def test_back_to_back_calls_without_sync(nchan, mode):
+    """Consecutive launches of the persistent kernel overlap (programmatic dependent launch) and hand the filter
+    history from one to the next inside the kernels: six calls of 7..12 blocks queued with no read and no
+    synchronisation in between, from an idle GPU, five times over; results must match the oracle every time."""
+    torch, sp = _torch(), _sp()
+    T = 8 if mode == PFB else 1
+    M = 11
+    sizes = [9, 7, 12, 8, 10, 7]
+    nblk = sum(sizes)
+    raw = synth.dual_pol_stream(700 + nchan // 1024 + mode, nblk * nchan, [synth.F_CFG1])
+    r, rd = oracle_run(raw, nchan, T, 2, mode, M, window=(1 if mode == PFB else 0))
+    d = torch.from_numpy(raw.reshape(-1)).cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    s = sp.Spec(nchan, T, 2, mode, M, 1 if mode == PFB else 0)
+    s.set_ring(16)
+    for rep in range(5):
+        torch.cuda.synchronize()
+        pos = 0
+        for n in sizes:
+            s.process(d.data_ptr() + pos * nchan * 4, n * nchan, st)
+            pos += n
+        assert s.spectra_done() == rd
+        outs = []
+        while s.pending():
+            outs.append(s.read_accum_host(st))
+        assert len(outs) == len(r)
+        for a, b in zip(outs, r):
+            compare(a, b, f"back-to-back N={nchan} mode={mode} rep={rep}")
+        s.reset()
+    s.close()
+
+
+def test_soak_random_call_sizes_two_handles_and_a_foreign_kernel():
+    """More than 200 back-to-back launches per handle with random call sizes (some shorter than the T-1 = 7
+    blocks of history, so both history-carry paths alternate), two handles on two streams, and a foreign kernel
+    that takes every SM's shared memory for 50 ms in the middle of it on a third stream."""
+    torch, sp = _torch(), _sp()
+    cfgs = [(8192, PFB, 8, 97), (32768, FFT, 1, 64), (1024, PFB, 8, 500)]
+    rng = np.random.default_rng(2026)
+    ncalls = 220
+    plans, raws, specs, devs = [], [], [], []
+    for i, (N, mode, T, M) in enumerate(cfgs):
+        sizes = rng.integers(1, 25, size=ncalls)
+        sizes[rng.integers(0, ncalls, size=40)] = rng.integers(1, 7, size=40)   # plenty of calls below T-1 blocks
+        plans.append(sizes)
+        raws.append(synth.dual_pol_stream(1200 + i, int(sizes.sum()) * N, [synth.F_CFG1]))
+        specs.append(sp.Spec(N, T, 2, mode, M, 1 if mode == PFB else 0))
+        specs[-1].set_ring(64)
+        devs.append(torch.from_numpy(raws[-1].reshape(-1)).cuda())
+    streams = [torch.cuda.Stream() for _ in cfgs]
+    hog_stream = torch.cuda.Stream()
+    outs = [[] for _ in cfgs]
+    pos = [0] * len(cfgs)
+    torch.cuda.synchronize()
+    for c in range(ncalls):
+        for i, (N, mode, T, M) in enumerate(cfgs):
+            n = int(plans[i][c])
+            specs[i].process(devs[i].data_ptr() + pos[i] * N * 4, n * N, streams[i].cuda_stream)
+            pos[i] += n
+            if specs[i].pending() > 40:      # drain now and then (the only reads; no other synchronisation)
+                while specs[i].pending():
+                    outs[i].append(specs[i].read_accum_host(streams[i].cuda_stream))
+        if c == ncalls // 2:
+            sp.debug_hog(50, 200 * 1024, hog_stream.cuda_stream)
+    for i in range(len(cfgs)):
+        while specs[i].pending():
+            outs[i].append(specs[i].read_accum_host(streams[i].cuda_stream))
+        specs[i].close()
+    torch.cuda.synchronize()
+    for i, (N, mode, T, M) in enumerate(cfgs):
+        r, _ = oracle_run(raws[i], N, T, 2, mode, M, window=(1 if mode == PFB else 0))
+        assert len(outs[i]) == len(r) and len(r) >= 2
+        for a, b in zip(outs[i], r):
+            compare(a, b, f"soak N={N}")
+
+
+# ---------------------------------------------------------------- configs[4]: the sweep's accumulation lengths
+
+SWEEP_LOG2 = 26          # samples per point here; configs[4] runs 2^31 (bench.py --sweep), same M/N ratio per sample
+SWEEP_POINTS = [(n, m) for m in (FFT, PFB) for n in (1 << k for k in range(10, 20))]
+
+
+@pytest.fixture(scope="module")
+def sweep_refs():
+    """One 2^26-sample config-1 stream and the oracle's accumulation for every sweep point: nacc = 2^26/N
+    (minus 7 for the PFB), one complete window each, computed in parallel processes."""
+    import os
+    ns = 1 << SWEEP_LOG2
+    path, raw = make_stream_file(synth.SEED_BASE + 4, ns)
+    jobs = []
+    for n, m in SWEEP_POINTS:
+        T = 8 if m == PFB else 1
+        jobs.append((n, T, 2, m, ns // n - (T - 1), 1 if m == PFB else 0))
+    res = oracle_many(path, ns, jobs)
+    yield raw, {pt: r for pt, r in zip(SWEEP_POINTS, res)}
+    del raw
+    os.unlink(path)
+
+
+@pytest.mark.parametrize("nchan,mode", SWEEP_POINTS)
+def test_sweep_accumulation_lengths(sweep_refs, nchan, mode):
+    """configs[4] at its real accumulation lengths per sample (M = 65536 at N=1024 ... 128 at N=524288 over 2^26
+    samples), fed in 64 MiB calls like bench.py does; every other point goes through spec_stream_host."""
+    torch, sp = _torch(), _sp()
+    raw, refs = sweep_refs
+    outs_ref, done_ref = refs[(nchan, mode)]
+    ns = 1 << SWEEP_LOG2
+    T = 8 if mode == PFB else 1
+    M = ns // nchan - (T - 1)
+    assert len(outs_ref) == 1 and done_ref == M
+    streamed = (SWEEP_POINTS.index((nchan, mode)) % 2 == 1)
+    st = torch.cuda.current_stream().cuda_stream
+    s = sp.Spec(nchan, T, 2, mode, M, 1 if mode == PFB else 0)
+    chunk = 1 << 24
+    if streamed:
+        hp = torch.from_numpy(np.asarray(raw).reshape(-1)).pin_memory()
+        assert s.stream_host(hp.data_ptr(), ns, chunk, st) == 1
+    else:
+        d = torch.from_numpy(np.asarray(raw).reshape(-1)).cuda()
+        done = 0
+        for c in range(ns // chunk):
+            done += s.process(d.data_ptr() + c * chunk * 4, chunk, st)
+        assert done == 1
+    got = s.read_accum_host(st)
+    assert s.spectra_done() == M
+    s.close()
+    w = compare(got, outs_ref[0], f"sweep N={nchan} mode={mode} M={M} streamed={streamed}")
+    check_stokes_invariants(got)
+    assert w["rel_l2"] < 3e-5      # far inside the 1e-4 tolerance: no drift from the accumulation length
+
+
+def test_sweep_longest_accumulation_2e21_spectra(sweep_refs):
+    """SURVEY 8(c) A18 / configs[4] at N=1024 direct FFT: M = 2^21 spectra, 2^31 samples.  The device-resident
+    2^26-sample buffer is fed 32 times (direct-FFT mode has no memory between blocks, so the accumulation is
+    exactly 32 times the oracle's sum over the 2^16 spectra of the buffer, computed in fp64)."""
+    torch, sp = _torch(), _sp()
+    raw, refs = sweep_refs
+    outs_ref, _ = refs[(1024, FFT)]
+    N, M, reps = 1024, 1 << 21, 32
+    st = torch.cuda.current_stream().cuda_stream
+    d = torch.from_numpy(np.asarray(raw).reshape(-1)).cuda()
+    s = sp.Spec(N, 1, 2, FFT, M, 0)
+    chunk = 1 << 24
+    done = 0
+    for rep in range(reps):
+        for c in range((1 << SWEEP_LOG2) // chunk):
+            done += s.process(d.data_ptr() + c * chunk * 4, chunk, st)
+    assert done == 1 and s.spectra_done() == M
+    got = s.read_accum_host(st)
+    s.close()
+    w = compare(got, reps * np.asarray(outs_ref[0]), "N=1024 FFT M=2^21")
+    assert w["rel_l2"] < 3e-5
 
 
 # ---------------------------------------------------------------- BASELINE.json configs
