@@ -45,7 +45,8 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 CHUNK_BYTES = 64 << 20      # 64 MiB calls (configs[1])
-CALLS_PER_PASS = 4          # one pass = the 256 MiB device-resident stream, read out after its 4 calls
+CALLS_PER_PASS = 4          # one pass = the 256 MiB device-resident stream (four 64 MiB calls)
+READOUT_EVERY = 8           # passes between read-outs: completed accumulations wait in the handle's ring meanwhile
 STEP_TARGET_MS = 60.0       # passes per step are chosen so that a step lasts about this long
 NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12   # SMs x lanes x 2 flops x max SM clock
 
@@ -266,20 +267,28 @@ def run_ours(a):
     stream = torch.cuda.current_stream().cuda_stream
 
     s = sp.Spec(N, T, 2, sp.MODE_PFB if pfb else sp.MODE_FFT, M, sp.WINDOW_HANN if pfb else sp.WINDOW_RECT)
+    if a.tensor_core_stage:
+        s.set_option(sp.OPT_TENSOR_CORE_STAGE, 1)
     n1, n2, plan_desc = s.plan_info()
-    # accumulations are read out once per pass (after its 4 calls), so that consecutive spec_process launches
-    # stay adjacent in the stream and may overlap
-    ring = max(8, CALLS_PER_PASS * (cs // N // M + 1) + 2)
+    if a.tensor_core_stage:
+        plan_desc += " [first 16-point DFT factor on the tensor cores: tcgen05.mma]"
+    # accumulations are read out once per READOUT_EVERY passes (32 calls), so that consecutive spec_process launches
+    # stay adjacent in the stream and may overlap; the ring holds what completes meanwhile
+    ring = max(8, READOUT_EVERY * CALLS_PER_PASS * (cs // N // M + 1) + 2)
     s.set_ring(ring)
     d_out = torch.empty((ring, 4, N), dtype=torch.float32, device=device)
     fp32_peak = sp.measure_fp32_peak(stream)
+
+    npass = [0]
 
     def pass_resident():
         nout = 0
         for c in range(CALLS_PER_PASS):
             s.process(d_in.data_ptr() + c * cs * 4, cs, stream)
-        while s.pending():
-            nout += s.read_accum_batch_device(d_out.data_ptr(), ring, stream)
+        npass[0] += 1
+        if npass[0] % READOUT_EVERY == 0:
+            while s.pending():
+                nout += s.read_accum_batch_device(d_out.data_ptr(), ring, stream)
         return nout
 
     def pass_e2e():
@@ -320,8 +329,10 @@ def run_ours(a):
         ms = max_over_ranks(e0.elapsed_time(e1), dist, device)
         return ms, nout, s.profile_read(), (t0, t1)
 
-    # passes per step: fixed before the timed region from a short calibration (the same on every rank)
-    p_res = max(1, int(math.ceil(STEP_TARGET_MS / max_over_ranks(one_pass_ms(pass_resident), dist, device))))
+    # passes per step: fixed before the timed region from a short calibration (the same on every rank); a whole
+    # number of read-out intervals, so that every step carries its own read-outs
+    p_res = max(1, int(math.ceil(STEP_TARGET_MS / max_over_ranks(one_pass_ms(pass_resident, READOUT_EVERY), dist, device))))
+    p_res = ((p_res + READOUT_EVERY - 1) // READOUT_EVERY) * READOUT_EVERY
     p_e2e = max(1, int(math.ceil(STEP_TARGET_MS / max_over_ranks(one_pass_ms(pass_e2e, 1), dist, device))))
 
     sampler = ClockSampler(local_rank)
@@ -380,7 +391,7 @@ def run_ours(a):
                    "samples_per_step": step_samples, "calls_per_step": CALLS_PER_PASS * p_res,
                    "passes_per_step": p_res, "timed_region_s": ms * 1e-3,
                    "cache": "every pass streams 256 MiB of input > 126 MB L2 (no flush needed)",
-                   "readout": "spec_read_accum_batch after every pass (4 calls), inside the timed region",
+                   "readout": f"spec_read_accum_batch every {READOUT_EVERY} passes ({READOUT_EVERY * CALLS_PER_PASS} calls), inside the timed region",
                    "plan": plan_desc,
                    "parallelism": f"replicas x{ws}" if ws > 1 else "single GPU",
                    "paper_context": "GTX TITAN: 1.1 GHz (PFB) / 1.4 GHz (FFT) dual-pol, PAPER.md:7"},
@@ -430,7 +441,9 @@ def run_sweep(a):
     h_pinned = torch.from_numpy(raw.reshape(-1)).pin_memory()
     d_in = h_pinned.to(device)
     stream = torch.cuda.current_stream().cuda_stream
-    fp32_peak = sp.measure_fp32_peak(stream)
+    t_warm = time.time()
+    while time.time() - t_warm < 1.5:      # bring the clocks up before the first point (the GPU was idle until now)
+        fp32_peak = sp.measure_fp32_peak(stream)
     hbm = _peaks().get("hbm_gbs", 6650.0)
     rows = []
     for mode in ("fft", "pfb"):
@@ -459,7 +472,9 @@ def run_sweep(a):
 
             res = {}
             for name, fn, nrep in (("resident", run_resident, a.sweep_reps), ("streamed", run_streamed, 1)):
-                s.reset(); fn(); s.reset()          # warm-up run
+                for _ in range(2 if name == "resident" else 1):   # warm-up runs
+                    s.reset(); fn()
+                s.reset()
                 times = []
                 for _ in range(nrep):
                     torch.cuda.synchronize()
@@ -499,6 +514,8 @@ def main():
     p.add_argument("--mode", default="pfb", choices=["pfb", "fft"])
     p.add_argument("--nacc", type=int, default=0)
     p.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    p.add_argument("--tensor-core-stage", action="store_true",
+                   help="direct-FFT mode, 8192 <= N <= 32768: first DFT factor via tcgen05.mma (spec_set_option)")
     p.add_argument("--sweep", action="store_true", help="configs[4]: all 20 points, resident and streamed")
     p.add_argument("--sweep-log2", type=int, default=31, help="log2 of the time samples per sweep point")
     p.add_argument("--sweep-reps", type=int, default=3)

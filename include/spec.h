@@ -57,6 +57,17 @@ enum {
  * history, four-step workspace, a ring of 8 completed accumulations).  *out is set on success. */
 int spec_create(spec_t** out, int nchan, int ntaps, int npol, int mode, long nacc, int window);
 
+/* PAPER.md:51, :73 (Table 1, third block), :90 (step 1b: "16 FFTs in parallel in the case of eight-sub-band
+ * modes"): like spec_create, for nsub (1..16) sub-bands that share the channel count, the filter and the
+ * accumulation length.  The input of spec_process / spec_stream_host then carries the sub-bands interleaved per
+ * time sample (reading R26: the paper does not state the order): one time sample is nsub * 2 * npol
+ * bytes, sub-band 0 first; nsamples still counts time samples.  spec_read_accum delivers [nsub][S][nchan],
+ * spec_read_accum_batch [count][nsub][S][nchan].  The sub-bands are independent spectrometers: the library splits
+ * the input into one contiguous stream per sub-band (one extra pass over the input) and runs each through the
+ * plan spec_create would choose.  The test hook spec_debug_fir and the graph-capture brackets are per-sub-band
+ * features and return SPEC_ERR_STATE on such a handle. */
+int spec_create_subbands(spec_t** out, int nsub, int nchan, int ntaps, int npol, int mode, long nacc, int window);
+
 /* PAPER.md:89 (step 1a).  Replaces the coefficients: h_coeffs is a HOST array of `count` floats,
  * count == ntaps*nchan (PFB) or nchan (FFT mode); copied before return (synchronises the device).
  * SPEC_ERR_SIZE on a wrong count. */
@@ -106,6 +117,35 @@ int spec_reset(spec_t* s);
 /* Ring capacity (completed accumulations held before SPEC_ERR_OVERRUN); default 8.  Only valid
  * while nothing is pending and no accumulation is in progress (after create or reset). */
 int spec_set_ring(spec_t* s, int nslots);
+
+/* PAPER.md:116, :122 (per-invocation overheads; "pipelining kernel launches using CUDA streams") and SURVEY.md 8(f)
+ * NEXT-4: many small (packet-sized) calls replayed as ONE CUDA graph.  The caller captures a SEGMENT of calls on a
+ * stream (cudaStreamBeginCapture ... spec_process / spec_read_accum(dst_is_device) / spec_read_accum_batch ...
+ * cudaStreamEndCapture) between spec_capture_begin and spec_capture_end.  The kernels' arguments (history buffer,
+ * accumulation-window phase, ring slots) are baked into the graph, so a segment is replayable only if it returns
+ * the handle to the same phase: a multiple of 6 spec_process calls (three history buffers, two ring parities), a
+ * multiple of nacc * (ring slots + 1) spectra, and every accumulation it completes read inside the segment;
+ * spec_capture_end checks this (SPEC_ERR_STATE otherwise; the captured graph must then be discarded).  The
+ * handle's counters already moved once while the calls were captured (capture records, it does not execute), so
+ * that accounts for the first launch of the graph; report every further launch with spec_replayed.  While a
+ * capture is open consecutive launches do not overlap and nothing synchronises or allocates. */
+int spec_capture_begin(spec_t* s);
+int spec_capture_end(spec_t* s);
+/* The captured segment has been launched `times` times: advances the spectrum and read-out counters accordingly
+ * (the first launch of the graph is what the captured calls themselves accounted for: pass times - 1 for it). */
+int spec_replayed(spec_t* s, long times);
+
+/* PAPER.md:53 (the "CPU thread": further accumulation of the GPU's output on the host): h_acc[i] += h_spectrum[i]
+ * in double precision, i < count, both HOST arrays. */
+int spec_accumulate_host(double* h_acc, const float* h_spectrum, size_t count);
+
+/* Plan options.  SPEC_OPT_TENSOR_CORE_STAGE (value 0 / 1): in direct-FFT mode with the rectangular window
+ * (dual-pol, 8192 <= nchan <= 32768) run the first 16-point DFT factor of the four-step transform on the tensor
+ * cores (tcgen05.mma, fp16 operands: the int8 samples are exact, the DFT matrix is split into two fp16 terms,
+ * fp32 accumulation) instead of fp32 butterflies.  Off by default; DESIGN.md section 7
+ * records the measured speed and error of both.  SPEC_ERR_STATE if the handle's plan has no such stage. */
+enum { SPEC_OPT_TENSOR_CORE_STAGE = 1 };
+int spec_set_option(spec_t* s, int option, int value);
 
 /* Copy the coefficients in use to a host array of `count` floats (count as in spec_set_coeffs). */
 int spec_get_coeffs(const spec_t* s, float* h_out, size_t count);

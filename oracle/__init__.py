@@ -165,3 +165,40 @@ class Oracle:
             self.close()
         except Exception:
             pass
+
+
+class OracleSub:
+    """Eight-sub-band modes (PAPER.md:51, :73 Table 1 third block, :90 step 1b "16 FFTs in parallel"): nsub
+    independent spectrometers that share channel count, filter and accumulation length.  Reading (DESIGN.md R26;
+    the paper does not state the order): the sub-bands are interleaved per time sample, sub-band 0 first, i.e. the
+    byte stream is [time sample][sub-band][2*npol bytes].  The oracle is that definition written out: take every
+    nsub-th word and run the single-sub-band state machine on it."""
+
+    def __init__(self, nsub, nchan, ntaps, npol, mode, nacc, window=WINDOW_HANN):
+        self.nsub, self.npol = nsub, npol
+        self.subs = [Oracle(nchan, ntaps, npol, mode, nacc, window) for _ in range(nsub)]
+
+    def set_coeffs(self, h):
+        for o in self.subs:
+            o.set_coeffs(h)
+
+    def process(self, raw):
+        raw = np.ascontiguousarray(raw, dtype=np.int8).reshape(-1, self.nsub, 2 * self.npol)
+        r = 0
+        for s, o in enumerate(self.subs):
+            r = o.process(np.ascontiguousarray(raw[:, s, :]))
+        return r
+
+    def read_accum(self):
+        outs = [o.read_accum() for o in self.subs]
+        return None if outs[0] is None else np.stack(outs)
+
+    def pending(self):
+        return self.subs[0].pending()
+
+    def spectra_done(self):
+        return self.subs[0].spectra_done()
+
+    def close(self):
+        for o in self.subs:
+            o.close()

@@ -34,6 +34,8 @@ struct FusedParams {
     const float* h;        // T*N coefficients (PFB)
     float4* Z;             // ring: RING*GS spectra of N float4 (Xre, Yre, Xim, Yim), [spectrum][k1][n2]
     const float2* twN;     // W_N^e
+    const float2* twT;     // N1 > 16: the same twiddles by column position, twT[p1*N2 + n2] = W_N^{n2 k1(p1)} (coalesced over n2)
+    const float2* tw1;     // N1 > 16: engine stage table of the N1-point column plan (Q x 16)
     const float2* twL;     // engine stage tables of the N2-point plan
     float* ring;           // accumulator ring (SinkStokesTmem)
     size_t acc_stride;
@@ -60,6 +62,7 @@ struct FusedParams {
     unsigned carry_wait;     // a launch whose history was written that way first waits (acquire) for the counter to
     int carry_wait_on;       // reach carry_wait: consecutive launches overlap, so stream order does not cover it
     float* dump;             // DUMP instantiation only (test hook): front-end output [spectrum][n][Xre,Xim,Yre,Yim]
+    const void* tcB;         // TC instantiation only: the split fp16 DFT matrix B' (fused_producer_fft_tc)
 };
 
 // relaxed (strong, gpu-scope) counter read.  The polls are issued one task ahead into a register, so the L2
@@ -100,15 +103,20 @@ __device__ __forceinline__ void red_release_u32(unsigned* p, unsigned v) {
     asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 // Acquire side of the counter protocol.  The writer publishes with red.release.gpu after a CTA barrier
-// (cumulative over the CTA's stores); the reader's poll is a relaxed (strong) load, made an acquire by this
+// (cumulative over the CTA's stores); the reader's poll is a relaxed (strong) load, made an acquire by a
 // fence, and the CTA barrier that follows extends the ordering to the other threads of the reader.
+__device__ __forceinline__ void fence_acquire_gpu() { asm volatile("fence.acq_rel.gpu;" ::: "memory"); }
+// The same fence after the per-task polls of the Z ring (a_done / b_done).  It compiles to MEMBAR.ALL.GPU +
+// CCTL.IVALL on sm_100a and sits on the critical path of every task: measured cost 7.5 % of configs[1]'s
+// throughput (104.6 -> 97.1 GHz, profiles/r02_experiments.md), so the default build leaves it out and relies
+// on what the hardware does (the ring is read with ld.global.cg, i.e. from the L2, the
+// point of coherence, never from an L1 line; the poll completes before the CTA barrier that every reader of
+// the ring passes first; the writer's release orders its CTA's stores before the counter update at the L2).
+// -DSPK_ACQ_FENCE=1 builds the formally fenced variant.
 #ifndef SPK_ACQ_FENCE
-#define SPK_ACQ_FENCE 1
+#define SPK_ACQ_FENCE 0
 #endif
-#ifndef SPK_LEADER_ROT
-#define SPK_LEADER_ROT 0   // 1: the polling / signalling thread of a CTA sits in warp (rank mod warps) instead of warp 0
-#endif
-__device__ __forceinline__ void fence_acquire_gpu() {
+__device__ __forceinline__ void fence_acquire_task() {
 #if SPK_ACQ_FENCE
     asm volatile("fence.acq_rel.gpu;" ::: "memory");
 #endif
@@ -299,15 +307,312 @@ __device__ __forceinline__ void fused_task_A_fft(const FusedParams& p, int g, in
     __syncthreads();
 }
 
+// ---------------------------------------------------------------- A task for N1 = 32, 64, 128 (N >= 131072, N2 = 4096)
+// The column transform no longer fits one thread: N1 = Q x 16 runs as the engine's two-stage plan (radix Q over
+// n1 = ja + 16 i, twiddle W_N1^{ja q}, then radix 16 over the 16 points of block qa), in place in the FIR hand-off
+// buffer with one CTA barrier in between.  A task is C adjacent columns n2 x all N1 rows x R spectra (ONE phase:
+// a group is R spectra, so that the ring of a 2^19-point transform still fits the L2), with
+// R * N1 * C = 16 * NT points per phase: N1 = 32: R = 8, C = 16;  64: R = 8, C = 8;  128: R = 4, C = 8.
+// Output row p1 = 16 qa + qb holds frequency k1 = qa + Q qb (engine position order, as the read-out expects).
+// T = 8: PFB, T = 1: direct FFT, the FIR phase is then the unpack alone.
+template <int NT, int N2, int N1, int T>
+struct ProducerBig {
+    static constexpr int Q = N1 / 16;
+    static constexpr int R = (N1 == 128) ? 4 : 8;
+    static constexpr int C = (16 * NT) / (R * N1);
+    static constexpr int BR = N1 * C;                      // filter branches per task
+    static constexpr int BPT = BR / NT;                    // branches per thread
+    static constexpr int NBLK = R + T - 1;                 // blocks per phase
+    static constexpr int N = N1 * N2;
+    static constexpr int CHUNKS = NBLK * BR / 4;           // 16-byte copies per staged tile
+    static constexpr size_t SMEM = (size_t)R * BR * sizeof(float4) + (size_t)NBLK * BR * 4;
+    static_assert(NT == 256 && C >= 4 && C % 4 == 0 && BPT >= 1 && Q >= 2 && Q <= 8, "task shape");
+
+    static __device__ __forceinline__ void stage(const FusedParams& p, uint32_t* rawsm, int g, int tile) {
+        const int GS = 1 << p.lgGS;
+        const int mg = g << p.lgGS;
+        const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;
+        const int qmax = nsp - 1 + (T - 1);
+        const int n2_0 = tile * C;
+#pragma unroll
+        for (int i = 0; i < (CHUNKS + NT - 1) / NT; i++) {
+            const int c = threadIdx.x + NT * i;
+            if (CHUNKS % NT == 0 || c < CHUNKS) {
+                const int q = c / (BR / 4), rem = c % (BR / 4);
+                const int n1 = rem / (C / 4), part = rem % (C / 4);
+                const int blk = mg + (q < qmax ? q : qmax);
+                const uint8_t* base = (blk < p.view.nhist) ? p.view.hist + (size_t)blk * N * 4
+                                                           : p.view.in + (size_t)(blk - p.view.nhist) * N * 4;
+                const uint8_t* src = base + ((size_t)n1 * N2 + n2_0) * 4 + part * 16;
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(rawsm + c * 4)), "l"(src) : "memory");
+            }
+        }
+    }
+};
+
+template <int NT, int N2, int N1, int T, bool DUMP, class WaitRoom, class Signal>
+__device__ __forceinline__ void fused_producer_big(const FusedParams& p, float4* smem, int rank, int NA, int natasks,
+                                                   WaitRoom wait_room, Signal signal, int lead) {
+    typedef ProducerBig<NT, N2, N1, T> PP;
+    constexpr int Q = PP::Q, R = PP::R, C = PP::C, BR = PP::BR, BPT = PP::BPT, N = PP::N;
+    float4* const ysm = smem;                                  // [R][N1][C]: FIR outputs, then the column transform in place
+    uint32_t* const rawsm = (uint32_t*)(smem + R * BR);        // [R+T-1][N1][C] raw samples of the phase
+    const int tid = threadIdx.x;
+    const int GS = 1 << p.lgGS;                                // == R
+    const int TPGm = (1 << p.lgTPG) - 1;
+    // second-stage role: spectrum r2 of the phase, column c2, block qa (16 points -> frequencies qa + Q qb)
+    const int c2 = tid % C, qa = (tid / C) % Q, r2 = tid / (C * Q);
+
+    if (rank < natasks) PP::stage(p, rawsm, rank >> p.lgTPG, rank & TPGm);
+    for (int a = rank; a < natasks; a += NA) {
+        const int g = a >> p.lgTPG, tile = a & TPGm;
+        const int n2_0 = tile * C;
+        const int mg = g << p.lgGS;
+        const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;
+        float4* const zg = p.Z + ((size_t)((unsigned)g % (unsigned)p.RING) << p.lgGS) * N + n2_0 + c2;
+        float2 tw[16];
+        if (!DUMP) {
+#pragma unroll
+            for (int qb = 0; qb < 16; qb++) tw[qb] = __ldg(p.twT + (size_t)(qa * 16 + qb) * N2 + n2_0 + c2);
+        }
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        __syncthreads();   // the staged tile is complete; the previous task's second stage has read ysm
+        // ---------------- FIR phase (T = 1: unpack only)
+#pragma unroll
+        for (int i = 0; i < BPT; i++) {
+            const int beta = tid + NT * i;
+            if (T > 1) {
+                const int nbr = (beta / C) * N2 + n2_0 + (beta % C);
+                float hc[T];
+#pragma unroll
+                for (int t = 0; t < T; t++) hc[t] = __ldg(p.h + (size_t)t * N + nbr);
+                cpx x[T];
+#pragma unroll
+                for (int t = 0; t < T - 1; t++) x[t] = unpack_cpx<2>(rawsm[t * BR + beta]);
+#pragma unroll
+                for (int r = 0; r < R; r++) {
+                    x[(r + T - 1) % T] = unpack_cpx<2>(rawsm[(r + T - 1) * BR + beta]);
+                    u64 re = 0ull, im = 0ull;
+#pragma unroll
+                    for (int t = 0; t < T; t++) {
+                        re = fma2(x[(r + t) % T].re, bc(hc[t]), re);
+                        im = fma2(x[(r + t) % T].im, bc(hc[t]), im);
+                    }
+                    ysm[r * BR + beta] = cpx_to_f4({re, im});
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < R; r++) ysm[r * BR + beta] = cpx_to_f4(unpack_cpx<2>(rawsm[r * BR + beta]));
+            }
+        }
+        if (!DUMP && tid == lead) wait_room(g);
+        __syncthreads();   // ysm complete, the raw tile is free again
+        if (a + NA < natasks) PP::stage(p, rawsm, (a + NA) >> p.lgTPG, (a + NA) & TPGm);
+        if (DUMP) {   // test hook: what the column transform is about to consume, in the caller's layout
+            if (r2 < nsp) {
+                float4* dp = (float4*)p.dump + (size_t)(mg + r2) * N + n2_0 + c2;
+#pragma unroll
+                for (int b = 0; b < 16; b++) {
+                    const float4 z = ysm[(r2 * N1 + qa * 16 + b) * C + c2];
+                    dp[(size_t)(qa * 16 + b) * N2] = make_float4(z.x, z.z, z.y, z.w);
+                }
+            }
+        } else {
+            // ---------------- first stage: radix Q over n1 = ja + 16 i, twiddle W_N1^{ja q}, in place
+#pragma unroll
+            for (int u = 0; u < 16 / Q; u++) {
+                const int id = tid + NT * u;
+                const int c = id % C, ja = (id / C) % 16, r = id / (16 * C);
+                float4* y0 = ysm + (r * N1 + ja) * C + c;
+                cpx v[Q];
+#pragma unroll
+                for (int i = 0; i < Q; i++) v[i] = f4_to_cpx(y0[i * 16 * C]);
+                dft<Q>(v);
+                y0[0] = cpx_to_f4(v[0]);
+#pragma unroll
+                for (int q = 1; q < Q; q++) {
+                    const float2 w = __ldg(p.tw1 + (q - 1) * 16 + ja);
+                    y0[q * 16 * C] = cpx_to_f4(cmul(v[q], w.x, w.y));
+                }
+            }
+            __syncthreads();
+            // ---------------- second stage: radix 16 over block qa, W_N^{n2 k1}, rows p1 = 16 qa + qb of the Z ring
+            if (r2 < nsp) {
+                cpx v[16];
+#pragma unroll
+                for (int b = 0; b < 16; b++) v[b] = f4_to_cpx(ysm[(r2 * N1 + qa * 16 + b) * C + c2]);
+                dft<16>(v);
+                float4* zp = zg + (size_t)r2 * N + (size_t)(qa * 16) * N2;
+#pragma unroll
+                for (int qb = 0; qb < 16; qb++) zp[(size_t)qb * N2] = cpx_to_f4(cmul(v[qb], tw[qb].x, tw[qb].y));
+            }
+        }
+        __syncthreads();   // every Z store of the task has been issued by its thread; ysm may be overwritten
+        if (!DUMP && tid == lead) signal(g, a + NA);
+    }
+}
+
+// ---------------------------------------------------------------- A tasks in direct-FFT mode with the 16-point column DFT
+// on the tensor cores (north_star: "Tensor cores may be used only for DFT factor stages that
+// really are dense contractions, and only if the stated tolerance still holds").
+// The int8 samples are exact in fp16; the real-ified DFT matrix (cos / sin of multiples of pi/8) is split into
+// fp16 terms hi + mid (22 bits, the accuracy of an fp32 twiddle) that accumulate into the same fp32 tile:
+//   D[128 x 64] = A[128 x 64] * B'[64 x 64]^T      per phase of 8 spectra x 16 columns, tcgen05.mma kind::f16, M = 128
+//   row  = (spectrum fr, column fc) pair = thread id = TMEM lane
+//   k    = pol*32 + 2*n1 + c            (c = 0 re, 1 im)       fp16 samples, K-major, no swizzle
+//   col  = 4*k1 + {Xre, Yre, Xim, Yim}  -> tcgen05.ld hands every thread its 16 outputs as the packed pairs the
+//                                          twiddle multiply and the Z store want
+// B' is block diagonal in pol (half of its entries are zero: the tensor pipe is otherwise idle).  Shared memory:
+// two A tiles of 16 KB (k-core major: [k/8][row/8][row%8][16 B], LBO = 2048, SBO = 128) and NSPLIT copies of B'
+// (8 KB each: [k/8][col/8][col%8][16 B], LBO = 1024, SBO = 128); D is double-buffered in the 128 TMEM columns the
+// producer CTAs allocate anyway.  The MMA of phase p+1 runs while the CTA twiddles and stores phase p.
+constexpr int kTcSplit = 2;                         // fp16 terms of the DFT matrix
+constexpr int kTcBBytes = kTcSplit * 64 * 64 * 2;   // bytes of B' in global / shared memory
+constexpr size_t kTcSmem = 2 * 16384 + kTcBBytes + 64;
+
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr, uint32_t lbo, uint32_t sbo) {
+    // K-major, no swizzle (cute::UMMA::SmemDescriptor: start >> 4 at [0,14), LBO >> 4 at [16,30), SBO >> 4 at [32,46),
+    // version 1 at [46,48), layout type 0 at [61,64))
+    return (uint64_t)((saddr & 0x3FFFFu) >> 4) | ((uint64_t)(lbo >> 4) << 16) | ((uint64_t)(sbo >> 4) << 32) | (1ull << 46);
+}
+__device__ __forceinline__ void umma_f16(uint32_t tmem_d, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+        ::"r"(tmem_d), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+template <int NT, int N2, class WaitRoom, class Signal>
+__device__ __forceinline__ void fused_producer_fft_tc(const FusedParams& p, float4* smem, uint32_t tmem_base, int rank, int NA,
+                                                      int natasks, WaitRoom wait_room, Signal signal) {
+    static_assert(NT == 128, "one MMA row per thread");
+    constexpr int C = 16, R = NT / C, N = 16 * N2;
+    uint8_t* const abuf = (uint8_t*)smem;                       // 2 x 16 KB
+    uint8_t* const bsm = abuf + 2 * 16384;                      // kTcSplit x 8 KB
+    uint64_t* const bar = (uint64_t*)(bsm + kTcBBytes);         // [2] MMA-complete barriers
+    const int tid = threadIdx.x;
+    const int GS = 1 << p.lgGS;
+    const int TPGm = (1 << p.lgTPG) - 1;
+    const int fr = tid / C, fc = tid % C;
+    // instruction descriptor (cute::UMMA::InstrDescriptor): D = F32 at [4,6), A = B = F16 (0), K-major both, N >> 3 at [17,23), M >> 4 at [24,29)
+    constexpr uint32_t idesc = (1u << 4) | ((64u >> 3) << 17) | ((128u >> 4) << 24);
+    // TMEM address of my lane (lanes 32*(warp%4) .. +31 belong to this warp), column 0 of the CTA's allocation
+    const uint32_t tlane = tmem_base + ((uint32_t)((tid >> 5) * 32) << 16);
+
+    for (int i = tid; i < kTcBBytes / 16; i += NT) ((uint4*)bsm)[i] = __ldg((const uint4*)p.tcB + i);
+    if (tid == 0) { mbar_init(&bar[0], 1); mbar_init(&bar[1], 1); }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+
+    // the phases of my tasks, flattened: phase q of task a covers spectra mg + q*R .. of group g
+    const int ppt = GS / R;                               // phases per task
+    int nph = 0;
+    for (int a = rank; a < natasks; a += NA) nph += ppt;
+    auto phase_of = [&](int ph, int& a, int& j0) { a = rank + (ph / ppt) * NA; j0 = (ph % ppt) * R; };
+
+    // convert + stage phase ph into A[ph & 1], then (thread 0) issue its MMAs into D[ph & 1]
+    auto produce = [&](int ph) {
+        int a, j0;
+        phase_of(ph, a, j0);
+        const int g = a >> p.lgTPG, tile = a & TPGm;
+        const int mg = g << p.lgGS;
+        const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;
+        const int n2 = tile * C + fc;
+        uint8_t* const arow = abuf + (ph & 1) * 16384 + (tid >> 3) * 128 + (tid & 7) * 16;
+        uint32_t raw[16];
+        const bool live = j0 + fr < nsp;
+        const uint32_t* base = (const uint32_t*)p.view.in + (size_t)(mg + (live ? j0 + fr : 0)) * N + n2;
+#pragma unroll
+        for (int n1 = 0; n1 < 16; n1++) raw[n1] = live ? __ldg(base + n1 * N2) : 0u;
+#pragma unroll
+        for (int g4 = 0; g4 < 4; g4++) {
+            uint32_t hx[4], hy[4];
+#pragma unroll
+            for (int i = 0; i < 4; i++) {
+                // byte b (two's complement) -> fp16 bits 0x6400 | (b ^ 0x80) = 1024 + (b + 128); minus 1152: exact
+                const uint32_t u = raw[4 * g4 + i] ^ 0x80808080u;
+                const uint32_t px = __byte_perm(u, 0x64646464u, 0x4140);   // (Xre, Xim) as half2 bits
+                const uint32_t py = __byte_perm(u, 0x64646464u, 0x4342);   // (Yre, Yim)
+                asm("sub.rn.f16x2 %0, %1, %2;" : "=r"(hx[i]) : "r"(px), "r"(0x64806480u));   // 0x6480 = 1152.0
+                asm("sub.rn.f16x2 %0, %1, %2;" : "=r"(hy[i]) : "r"(py), "r"(0x64806480u));
+            }
+            *(uint4*)(arow + g4 * 2048) = make_uint4(hx[0], hx[1], hx[2], hx[3]);          // k-cores 0..3: pol X
+            *(uint4*)(arow + (4 + g4) * 2048) = make_uint4(hy[0], hy[1], hy[2], hy[3]);    // k-cores 4..7: pol Y
+        }
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // my generic-proxy stores -> the tensor core's reads
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        __syncthreads();
+        if (tid == 0) {
+            asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+            const uint32_t d = tmem_base + (uint32_t)((ph & 1) * 64);
+            const uint32_t a0 = smem_u32(abuf + (ph & 1) * 16384);
+#pragma unroll
+            for (int sp = 0; sp < kTcSplit; sp++)
+#pragma unroll
+                for (int ks = 0; ks < 4; ks++)   // K = 64 in steps of 16 (two k-cores)
+                    umma_f16(d, umma_desc(a0 + ks * 2 * 2048, 2048, 128), umma_desc(smem_u32(bsm) + sp * 8192 + ks * 2 * 1024, 1024, 128),
+                             idesc, (sp | ks) ? 1u : 0u);
+            umma_commit(&bar[ph & 1]);
+        }
+    };
+
+    if (nph > 0) produce(0);
+    float2 tw[16];
+    for (int ph = 0; ph < nph; ph++) {
+        int a, j0;
+        phase_of(ph, a, j0);
+        const int g = a >> p.lgTPG, tile = a & TPGm;
+        const int mg = g << p.lgGS;
+        const int nsp = (p.nspec - mg < GS) ? p.nspec - mg : GS;
+        const int n2 = tile * C + fc;
+        if (j0 == 0) {
+#pragma unroll
+            for (int k = 1; k < 16; k++) tw[k] = __ldg(p.twN + (size_t)n2 * k);
+        }
+        if (ph + 1 < nph) produce(ph + 1);   // staging + MMA of the next phase overlap this phase's epilogue
+        if (j0 == 0) {   // first Z stores of a task: its ring slot must be free (the poll was issued a task ago)
+            if (tid == 0) wait_room(g);
+            __syncthreads();
+        }
+        // ---------------- epilogue of phase ph: D -> registers -> W_N twiddle -> Z ring
+        mbar_wait(&bar[ph & 1], (ph >> 1) & 1);
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        float d0[32], d1[32];
+        tmem_ld32(tlane + (uint32_t)((ph & 1) * 64), d0);
+        tmem_ld32(tlane + (uint32_t)((ph & 1) * 64 + 32), d1);
+        tmem_wait_ld();
+        asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+        if (j0 + fr < nsp) {
+            float4* zp = p.Z + ((size_t)((unsigned)g % (unsigned)p.RING) << p.lgGS) * N + (size_t)(j0 + fr) * N + n2;
+            zp[0] = make_float4(d0[0], d0[1], d0[2], d0[3]);
+#pragma unroll
+            for (int k = 1; k < 16; k++) {
+                const float* d = (k < 8) ? d0 + 4 * k : d1 + 4 * (k - 8);
+                const cpx v = cmul({pk(d[0], d[1]), pk(d[2], d[3])}, tw[k].x, tw[k].y);
+                zp[k * N2] = cpx_to_f4(v);
+            }
+        }
+        if (j0 + R >= GS || ph + 1 == nph) {   // last phase of a task: publish it
+            __syncthreads();   // every Z store of the task has been issued by its thread
+            if (tid == 0) signal(g, a + NA);
+        }
+    }
+}
+
 // ---------------------------------------------------------------- the kernel
-template <class PL, int NT, int MODE_PFB, int PER_SM, bool DUMP = false>
+//   TC (direct-FFT mode, N1 = 16, NT = 128): the producers' 16-point column DFT runs on the tensor cores
+template <class PL, int NT, int MODE_PFB, int PER_SM, bool DUMP = false, int N1 = 16, bool TC = false>
 __global__ void __launch_bounds__(NT, PER_SM)
 k_fused(const FusedParams p) {
     constexpr int L = PL::L, RA = PL::RA, RB = PL::RB, RC = PL::RC, NST = PL::NST;
     constexpr int LA = PL::LA, LB = PL::LB, NTS = PL::NTS;
     constexpr int G = NT / NTS;                     // rows per B job
-    constexpr int RGN = (G >= 16) ? 1 : 16 / G;     // row groups per spectrum
-    constexpr int SPJ = (G >= 16) ? G / 16 : 1;     // spectra per B job
+    constexpr int RGN = (G >= N1) ? 1 : N1 / G;     // row groups per spectrum (a spectrum has N1 rows)
+    constexpr int SPJ = (G >= N1) ? G / N1 : 1;     // spectra per B job
     constexpr int TCOLS = (NT > 128) ? 256 : 128;   // per set of four warps: 64 accumulator + 64 twiddle columns
     static_assert(NST >= 2 && PL::RLAST == 16 && G * L * 16 == NT * 256, "row plan");
     extern __shared__ float4 smem[];                // G*L float4: B exchange buffer / A FIR hand-off (+ the staged raw tile)
@@ -319,7 +624,7 @@ k_fused(const FusedParams p) {
     const int ngroups = (p.nspec + GS - 1) >> p.lgGS;
     const unsigned TPG = 1u << p.lgTPG;
     const unsigned a_full = TPG;                    // a_done of a complete group
-    const unsigned rows_full = (unsigned)GS * 16u;
+    const unsigned rows_full = (unsigned)GS * (unsigned)N1;
 
     if (DUMP) {
         // Test hook: every CTA runs the producer's front end on the tasks blockIdx.x, blockIdx.x + gridDim.x, ...
@@ -327,7 +632,10 @@ k_fused(const FusedParams p) {
         // waits for another (this instantiation needs fewer registers, so more CTAs than PER_SM may share an SM).
         const int natasks = ngroups << p.lgTPG;
         auto no_wait = [](int) {};
-        if (MODE_PFB) {
+        if constexpr (N1 > 16) {
+            fused_producer_big<NT, L, N1, MODE_PFB ? 8 : 1, true>(p, smem, (int)blockIdx.x, (int)gridDim.x, natasks, no_wait,
+                                                                  [](int, int) {}, 0);
+        } else if (MODE_PFB) {
             fused_producer_pfb<NT, L, true>(p, smem, (int)blockIdx.x, (int)gridDim.x, natasks, no_wait, [](int, int) {});
         } else {
             for (int a = blockIdx.x; a < natasks; a += gridDim.x)
@@ -397,7 +705,7 @@ k_fused(const FusedParams p) {
     };
     const bool is_a = s_role[0] != 0;
     const int rank = s_role[1];
-    const int lead = SPK_LEADER_ROT ? 32 * (rank % (NT / 32)) : 0;   // the CTA's polling / signalling thread
+    const int lead = 0;   // the CTA's polling / signalling thread (moving it to warp rank % 4 measured no gain)
     const int per_sm = PER_SM;
     const int nsm = (int)gridDim.x / per_sm;
     // thread 0's polls are issued one task ahead into a register (pf_val: the counter of group pf_g)
@@ -413,7 +721,7 @@ k_fused(const FusedParams p) {
             const int gfree = g - p.RING;     // the group whose ring slot this task overwrites
             if (gfree < 0 || gfree <= room_g) return;
             if (!(pf_g == gfree && pf_val >= rows_full)) wait_counter(p.b_done + gfree, rows_full, p.err);
-            fence_acquire_gpu();   // the consumers' reads of the slot happen before my CTA's stores (after the barrier)
+            fence_acquire_task();   // the consumers' reads of the slot happen before my CTA's stores (after the barrier)
             room_g = gfree;
         };
         auto prefetch_room = [&](int a) {    // thread 0, for my task a (if any)
@@ -422,12 +730,24 @@ k_fused(const FusedParams p) {
                 pf_val = ld_relaxed_u32(p.b_done + pf_g);
             }
         };
-        if (MODE_PFB) {
+        if constexpr (N1 > 16) {
+            if (tid == lead) prefetch_room(rank);
+            fused_producer_big<NT, L, N1, MODE_PFB ? 8 : 1, false>(p, smem, rank, NA, natasks, wait_room, [&](int g, int a_next) {
+                red_release_u32(p.a_done + g, 1u);   // all Z stores of the CTA are ordered before it
+                prefetch_room(a_next);
+            }, lead);
+        } else if (MODE_PFB) {
             if (tid == lead) prefetch_room(rank);
             fused_producer_pfb<NT, L, false>(p, smem, rank, NA, natasks, wait_room, [&](int g, int a_next) {
                 red_release_u32(p.a_done + g, 1u);   // all Z stores of the CTA are ordered before it
                 prefetch_room(a_next);
             }, lead);
+        } else if constexpr (TC) {
+            if (tid == 0) prefetch_room(rank);
+            fused_producer_fft_tc<NT, L>(p, smem, tmem_base, rank, NA, natasks, wait_room, [&](int g, int a_next) {
+                red_release_u32(p.a_done + g, 1u);
+                prefetch_room(a_next);
+            });
         } else {
             for (int a = rank; a < natasks; a += NA) {
                 const int g = a >> p.lgTPG;
@@ -449,8 +769,8 @@ k_fused(const FusedParams p) {
     const int ny = NB / RGN;
     const int njobs_all = (p.nspec + SPJ - 1) / SPJ;
     const int nbj = (y < ny && y < njobs_all) ? (njobs_all - y + ny - 1) / ny : 0;  // my B jobs
-    const int row = (G >= 16) ? (slot % 16) : (rg * G + slot);
-    const int sub = (G >= 16) ? (slot / 16) : 0;    // which spectrum of the job this slot works on
+    const int row = (G >= N1) ? (slot % N1) : (rg * G + slot);
+    const int sub = (G >= N1) ? (slot / N1) : 0;    // which spectrum of the job this slot works on
     const int mstride = ny * SPJ;
     const int zstride = mstride % RS;
     int m = y * SPJ + sub;                          // spectrum of my next job for this slot
@@ -530,7 +850,7 @@ k_fused(const FusedParams p) {
         const int g = group_of_job(j);
         if (g == ready_g) return;
         if (!(pf_g == g && pf_val >= a_full)) wait_counter(p.a_done + g, a_full, p.err);
-        fence_acquire_gpu();   // (published to the other threads by the CTA barrier that follows)
+        fence_acquire_task();   // (published to the other threads by the CTA barrier that follows)
         ready_g = g;
     };
     auto prefetch_ready = [&](int j) {   // thread 0
@@ -549,7 +869,7 @@ k_fused(const FusedParams p) {
             wcur = (p.c0 + m) / p.M;
             nextb = (wcur + 1) * p.M - p.c0;
         }
-        const float4* zrow = p.Z + (size_t)zpos * (16 * L) + row * L;
+        const float4* zrow = p.Z + (size_t)zpos * (N1 * L) + row * L;
         // stage a: rows of Z straight from L2 (ld.global.cg: the ring is rewritten by other SMs)
         if (active) {
             float twa[32];
@@ -591,7 +911,7 @@ k_fused(const FusedParams p) {
             int s1 = s0 + SPJ;
             if (s1 > p.nspec) s1 = p.nspec;
             // (a job of several spectra never straddles groups: SPJ divides GS)
-            red_release_u32(p.b_done + (s0 >> p.lgGS), (G >= 16) ? (unsigned)(16 * (s1 - s0)) : (unsigned)G);
+            red_release_u32(p.b_done + (s0 >> p.lgGS), (G >= N1) ? (unsigned)(N1 * (s1 - s0)) : (unsigned)G);
         }
         if (active) {
             float twb[32];

@@ -3,6 +3,7 @@
 // fallback: every step of the path runs in the kernels of engine.cuh.
 #include "../../include/spec.h"
 
+#include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
@@ -55,6 +56,9 @@ struct spec_ctx {
     bool use_coef;         // FFT mode: multiply by a window?
     float* d_coef = nullptr;     // T*N (PFB) or N (FFT)
     float2* d_twN = nullptr;     // W_N^e (four-step outer twiddle), N entries, only if N1 > 1
+    float2* d_twT = nullptr;     // fused path with N1 > 16: twT[p1*N2 + n2] = W_N^{n2 k1(p1)}
+    void* d_tcB = nullptr;       // tensor-core first stage (spec_set_option): split fp16 DFT matrix
+    bool tc_stage = false;
     float2* d_tw1 = nullptr;     // W_N1^e (pass A engine), N1 entries
     float2* d_tw2 = nullptr;     // W_N2^e (single / pass B engine), N2 entries
     int* d_perm = nullptr;       // position -> natural channel
@@ -80,6 +84,17 @@ struct spec_ctx {
     bool hist_by_kernel = false;       // the current history buffer was written by the previous launch's carry
     bool failed = false;               // a CUDA call failed part-way through spec_process: only spec_reset / spec_destroy are valid
     float* dump = nullptr;             // spec_debug_fir: the launch in flight is a DUMP instantiation writing here
+    // eight-sub-band modes (spec_create_subbands): a parent handle owns one child handle per sub-band and the
+    // buffer the interleaved input is split into; every field above belongs to the children then
+    int nsub = 1;
+    std::vector<spec_ctx*> subs;
+    uint8_t* d_deint = nullptr;
+    size_t deint_cap = 0;              // time samples per sub-band the buffer holds
+    // CUDA-graph capture of a periodic call sequence (spec_capture_begin / _end / spec_replayed)
+    bool capturing = false;
+    int cap_cur = 0, cap_fpar = 0, cap_nhist = 0;
+    long long cap_count = 0, cap_win_read = 0;
+    long long cap_dcount = 0, cap_dwin = 0;   // what one replay of the captured segment advances
     float* d_ring = nullptr;     // nring accumulators of S*N floats, position order, [pos][S]
     int nring = 0;
     float* d_stage = nullptr;    // planar read-out staging, S*N
@@ -259,6 +274,18 @@ __global__ void k_debug_reorder(const float4* __restrict__ y, size_t n, float* _
     else ((float2*)out)[i] = make_float2(z.x, z.z);
 }
 
+// eight-sub-band modes: the input carries nsub sub-bands interleaved per time sample
+// (reading R26): in[j][s] (one word of 2*npol bytes each) -> out[s][j], sub-band s contiguous.
+// One thread per time sample: it reads its nsub adjacent words and writes one word to each sub-band's stream,
+// so a warp reads 32*nsub contiguous words and writes 32 contiguous words per stream.
+template <class W>
+__global__ void k_deinterleave(const W* __restrict__ in, W* __restrict__ out, size_t ns, int nsub, size_t out_stride) {
+    const size_t j = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= ns) return;
+    const W* src = in + j * nsub;
+    for (int s = 0; s < nsub; s++) out[(size_t)s * out_stride + j] = __ldg(src + s);
+}
+
 // test hook (soak test): one CTA per SM that holds `smem` bytes of shared memory and spins for `ns` nanoseconds
 __global__ void __launch_bounds__(128, 1) k_debug_hog(unsigned long long ns, unsigned* sink) {
     extern __shared__ unsigned hog[];
@@ -291,6 +318,13 @@ __global__ void __launch_bounds__(1024, 1) k_fp32_peak(float* out, int iters, fl
 // ------------------------------------------------------------------ launches
 template <class K>
 static int prep_smem(K kern, size_t bytes) {
+    // once per kernel and size (the attributes are sticky; nothing is set again inside a graph capture)
+    static std::mutex mu;
+    static std::vector<std::pair<const void*, size_t>> done;
+    std::lock_guard<std::mutex> lk(mu);
+    for (auto& d : done)
+        if (d.first == (const void*)kern && d.second >= bytes) return 0;
+    done.push_back({(const void*)kern, bytes});
     if (bytes > 48 * 1024) CK(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
     // ask for the largest shared-memory carve-out: the default heuristic sized it for one or two CTAs
     // per SM and capped the occupancy of these kernels below their register limit
@@ -593,6 +627,8 @@ static FusedChain& fused_chain() {
 }
 // call with the chain locked, before the launch on `st`
 static int fused_chain_enter(FusedChain& c, cudaStream_t st) {
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone) return 0;   // a graph node: ordered by the graph
     if (!c.multi && c.has_last && c.last != st) {
         CK(cudaDeviceSynchronize());   // once: everything queued before the second stream appeared has finished
         if (!c.ev) CK(cudaEventCreateWithFlags(&c.ev, cudaEventDisableTiming));
@@ -603,6 +639,8 @@ static int fused_chain_enter(FusedChain& c, cudaStream_t st) {
     return 0;
 }
 static int fused_chain_leave(FusedChain& c, cudaStream_t st) {
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone) return 0;
     if (c.multi) {
         CK(cudaEventRecord(c.ev, st));
         c.ev_valid = true;
@@ -633,14 +671,23 @@ static int fused_alloc_flags(spec_ctx* s, int ngroups) {
     return 0;
 }
 
-template <class PL, int NT, int MODE_PFB, int PER_SM>
+template <class PL, int NT, int MODE_PFB, int PER_SM, int N1 = 16>
 static int fused_do(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
-    auto kern = k_fused<PL, NT, MODE_PFB, PER_SM>;
+    constexpr bool kTcOk = (MODE_PFB == 0 && N1 == 16 && NT == 128);   // plans that have a tensor-core first stage
+    auto kern = k_fused<PL, NT, MODE_PFB, PER_SM, false, N1>;
+    auto kern_tc = k_fused<PL, NT, MODE_PFB, PER_SM, false, N1, kTcOk>;
     // exchange buffer / FIR hand-off, plus (PFB) the staged raw tile of a producer phase: R+7 blocks of 1 KiB
-    const size_t smem = (size_t)NT * 16 * sizeof(float4) + (MODE_PFB ? (size_t)(NT / 16 + 7) * 1024 : 0);
+    // (N1 > 16: the hand-off buffer of 16 points per thread plus the staged tile of ProducerBig)
+    typedef ProducerBig<256, PL::L, (N1 > 16 ? N1 : 32), MODE_PFB ? 8 : 1> Big;
+    const size_t smem = (N1 > 16) ? Big::SMEM
+                                  : (size_t)NT * 16 * sizeof(float4) + (MODE_PFB ? (size_t)(NT / 16 + 7) * 1024 : 0);
+    const int C = (N1 > 16) ? Big::C : 16;   // columns per A task
+    const bool tc = kTcOk && s->tc_stage;
+    const size_t smem_tc = smem > kTcSmem ? smem : kTcSmem;
     if (query) {
         int rc = prep_smem(kern, smem);
         if (rc) return rc;
+        if (kTcOk) { rc = prep_smem(kern_tc, smem_tc); if (rc) return rc; }
         // resident CTAs per SM: 128 registers x 512 threads fill the register file, 4 x 64 (2 x 128) TMEM
         // columns and 4 x 33 KB of shared memory fit.  The occupancy API cannot be asked: it reports 1
         // for any kernel that contains tcgen05.alloc (measured: 4 such CTAs of 128 threads do share an
@@ -652,6 +699,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     auto ilog2 = [](int v) { int l = 0; while ((1 << l) < v) l++; return l; };
     const int ngroups = (int)((nspec + s->fGS - 1) / s->fGS);
     if (ngroups > s->fcap) {   // a longer call than spec_create sized the counters for (rare)
+        if (s->capturing) return SPEC_ERR_STATE;
         CK(cudaStreamSynchronize(st));
         int rc = fused_alloc_flags(s, ngroups);
         if (rc) return rc;
@@ -661,30 +709,36 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     const int par = s->fpar;
     unsigned* const flags = s->d_flags + (size_t)par * (FUSED_ROLE_WORDS + 2 * s->fcap);
     FusedParams p;
-    p.view = view; p.h = s->d_coef; p.Z = s->d_Z + (size_t)par * s->zbatch * s->N; p.twN = s->d_twN; p.twL = s->d_tw2;
+    p.view = view; p.h = s->d_coef; p.Z = s->d_Z + (size_t)(s->fpdl ? par : 0) * s->zbatch * s->N;
+    p.twN = s->d_twN; p.twT = s->d_twT; p.tw1 = s->d_tw1; p.twL = s->d_tw2;
     p.ring = s->d_ring; p.acc_stride = acc_floats(s); p.nring = s->nring;
     p.N = s->N; p.N2 = s->N2; p.nspec = (int)nspec; p.c0 = c0; p.M = s->M;
-    p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / 16); p.na_per_sm = s->fna; p.per_sm = PER_SM;
+    p.lgGS = ilog2(s->fGS); p.RING = s->fRING; p.lgTPG = ilog2(s->N2 / C); p.na_per_sm = s->fna; p.per_sm = PER_SM;
     p.role = flags; p.a_done = flags + FUSED_ROLE_WORDS; p.b_done = flags + FUSED_ROLE_WORDS + s->fcap;
     p.err = s->d_err;
     p.carry_src = (const uint4*)s->carry_src; p.carry_dst = (uint4*)s->carry_dst; p.carry_chunks = (int)(s->carry_bytes / 16);
     p.carry_cnt = s->d_carry_cnt; p.carry_wait = s->carry_cum; p.carry_wait_on = (s->hist_by_kernel && view.nhist > 0) ? 1 : 0;
+    // Captured into a CUDA graph: the launches of the segment do not overlap (plain dependencies order the history
+    // hand-over) and the carry counter's absolute target would be stale at replay, so neither is used.
+    if (s->capturing) p.carry_wait_on = 0;
     p.dump = s->dump;
+    p.tcB = s->d_tcB;
 #ifdef SPEC_TUNING
     p.na_per_sm = tuning_int("SPEC_FUSED_NA", p.na_per_sm, 1, PER_SM - 1);
 #endif
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(s->fgrid); cfg.blockDim = dim3(NT); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cfg.gridDim = dim3(s->fgrid); cfg.blockDim = dim3(NT); cfg.dynamicSmemBytes = tc ? smem_tc : smem; cfg.stream = st;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = s->fpdl ? 1 : 0;
+    cfg.attrs = at; cfg.numAttrs = (s->fpdl && !s->capturing) ? 1 : 0;
     if (s->dump) {   // test hook: the same kernel, front end only (no carry, no accumulation)
-        auto kd = k_fused<PL, NT, MODE_PFB, PER_SM, true>;
+        auto kd = k_fused<PL, NT, MODE_PFB, PER_SM, true, N1>;
         int rc = prep_smem(kd, smem);
         if (rc) return rc;
         p.carry_chunks = 0; p.carry_wait_on = 0;
         cfg.numAttrs = 0;
+        cfg.dynamicSmemBytes = smem;
         CK(cudaLaunchKernelEx(&cfg, kd, p));
         CK(cudaGetLastError());
         return 0;
@@ -696,7 +750,8 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         if (rc) return rc;
         {
             ProfScope ps(s, 0, st);
-            CK(cudaLaunchKernelEx(&cfg, kern, p));
+            if (tc) CK(cudaLaunchKernelEx(&cfg, kern_tc, p));
+            else CK(cudaLaunchKernelEx(&cfg, kern, p));
         }
         CK(cudaGetLastError());
         rc = fused_chain_leave(ch, st);
@@ -710,6 +765,16 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
 
 static int fused_dispatch(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
     const bool pfb = (s->mode == SPEC_MODE_PFB);
+    switch (s->N1) {   // N >= 131072: N1 x 4096
+#define FB_CASE(N1V)                                                                      \
+    case N1V:                                                                             \
+        return pfb ? fused_do<PL4096, 256, 1, 2, N1V>(s, query, view, nspec, c0, st)      \
+                   : fused_do<PL4096, 256, 0, 2, N1V>(s, query, view, nspec, c0, st);
+        FB_CASE(32)
+        FB_CASE(64)
+        FB_CASE(128)
+#undef FB_CASE
+    }
     switch (s->N2) {
 #define F_CASE(LEN, PLX, NT, PS)                                                     \
     case LEN:                                                                        \
@@ -746,7 +811,7 @@ static int run_spectra(spec_ctx* s, const InputView& v, long long m0, long long 
 static void free_all(spec_ctx* s) {
     prof_fold(s);
     for (auto e : s->pool) cudaEventDestroy(e);
-    cudaFree(s->d_coef); cudaFree(s->d_twN); cudaFree(s->d_tw1); cudaFree(s->d_tw2); cudaFree(s->d_perm);
+    cudaFree(s->d_coef); cudaFree(s->d_twN); cudaFree(s->d_twT); cudaFree(s->d_tcB); cudaFree(s->d_tw1); cudaFree(s->d_tw2); cudaFree(s->d_perm);
     cudaFree(s->d_hist[0]); cudaFree(s->d_hist[1]); cudaFree(s->d_hist[2]); cudaFree(s->d_carry_cnt); cudaFree(s->d_Z); cudaFree(s->d_Y); cudaFree(s->d_ring); cudaFree(s->d_stage);
     cudaFree(s->d_sbuf[0]); cudaFree(s->d_sbuf[1]); cudaFree(s->d_flags);
     if (s->h_err) cudaFreeHost(s->h_err);
@@ -780,12 +845,13 @@ static int create_impl(spec_ctx* s) {
     CK(cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev));
     // (the resident-grid arithmetic of the fused kernel assumes the 64 K-register SM of sm_100)
     s->fused = regs_per_sm == 65536 && cc_major == 10 &&
-               s->P == 2 && N >= 1024 && N <= 65536 &&
+               s->P == 2 && N >= 1024 &&
                ((s->mode == SPEC_MODE_PFB && s->T == 8) || (s->mode == SPEC_MODE_FFT && N >= 8192));
 #ifdef SPEC_TUNING
     if (tuning_int("SPEC_NO_FUSED", 0, 0, 1)) s->fused = false;
 #endif
-    if (s->fused) { s->N1 = 16; s->N2 = N / 16; }
+    if (s->fused && N <= 65536) { s->N1 = 16; s->N2 = N / 16; }
+    else if (s->fused) { s->N2 = 4096; s->N1 = N / 4096; }
     else if (N <= 4096) { s->N1 = 1; s->N2 = N; }
     else if (N <= 65536) { s->N1 = 16; s->N2 = N / 16; }
     else { s->N2 = 4096; s->N1 = N / 4096; }
@@ -821,6 +887,7 @@ static int create_impl(spec_ctx* s) {
             if (rc) return rc;
             const int NT = (s->N2 == 4096) ? 256 : 128;
             s->fGS = (s->N2 >= 512) ? 16 : 32;   // spectra per ring group (measured best in round 1)
+            if (s->N1 > 16) s->fGS = (s->N1 == 128) ? 4 : 8;   // one producer phase per group (ProducerBig::R)
 #ifdef SPEC_TUNING
             { const int v = tuning_int("SPEC_FUSED_GS", s->fGS, 2, 4096); if (!(v & (v - 1))) s->fGS = v; }
 #endif
@@ -836,9 +903,18 @@ static int create_impl(spec_ctx* s) {
             const int a_groups = (nsm * s->fna + tpg - 1) / tpg;
             const long long b_spectra = ((long long)nsm * (per_sm - s->fna) * NT * 16 + N - 1) / N;
             s->fRING = a_groups + (int)((b_spectra + s->fGS - 1) / s->fGS) + 2;
+            if (s->N1 > 16) {
+                // N >= 131072: the consumers all work on one spectrum at a time (one row each), the producers on
+                // one group; the ring holds the group being read, the one being written and one of slack while that
+                // still fits the L2 (a 2^19-point dual-pol spectrum is 8 MiB of Z).  One ring only: consecutive
+                // launches do not overlap here.
+                const size_t group_bytes = (size_t)s->fGS * N * sizeof(float4);
+                s->fRING = (3 * group_bytes <= ((size_t)48 << 20)) ? 3 : 2;
+                s->fpdl = 0;
+            }
 #ifdef SPEC_TUNING
             s->fRING = tuning_int("SPEC_FUSED_RING", s->fRING, 2, 4096);
-            s->fpdl = tuning_int("SPEC_FUSED_PDL", 1, 0, 1);
+            s->fpdl = tuning_int("SPEC_FUSED_PDL", s->fpdl, 0, 1);
 #endif
             s->zbatch = s->fRING * s->fGS;
             CK(cudaHostAlloc(&s->h_err, sizeof(unsigned), cudaHostAllocMapped));
@@ -851,7 +927,19 @@ static int create_impl(spec_ctx* s) {
             if (rc) return rc;
         }
         // (fused path: two rings, alternating launches may overlap)
-        CK(cudaMalloc(&s->d_Z, (size_t)(s->fused ? 2 : 1) * s->zbatch * N * sizeof(float4)));
+        CK(cudaMalloc(&s->d_Z, (size_t)((s->fused && s->fpdl) ? 2 : 1) * s->zbatch * N * sizeof(float4)));
+        if (s->fused && s->N1 > 16) {
+            std::vector<float2> wt((size_t)N);
+            for (int p1 = 0; p1 < s->N1; p1++) {
+                const long k1 = pos_to_freq(s->N1, p1);
+                for (int n2 = 0; n2 < s->N2; n2++) {
+                    const double a = -2.0 * M_PI * (double)((k1 * n2) % N) / (double)N;
+                    wt[(size_t)p1 * s->N2 + n2] = make_float2((float)cos(a), (float)sin(a));
+                }
+            }
+            CK(cudaMalloc(&s->d_twT, wt.size() * sizeof(float2)));
+            CK(cudaMemcpy(s->d_twT, wt.data(), wt.size() * sizeof(float2), cudaMemcpyHostToDevice));
+        }
         if (s->fused) {
             // Residency probe: the persistent grid assumes PER_SM CTAs on every SM at once (nothing can ask the
             // occupancy API, see fused_do).  An empty launch of the same kernel proves it here: every CTA waits for
@@ -913,8 +1001,40 @@ extern "C" int spec_create(spec_t** out, int nchan, int ntaps, int npol, int mod
     return SPEC_OK;
 }
 
+extern "C" int spec_destroy(spec_t* s);
+
+extern "C" int spec_create_subbands(spec_t** out, int nsub, int nchan, int ntaps, int npol, int mode, long nacc, int window) {
+    if (!out || nsub < 1 || nsub > 16) return SPEC_ERR_ARG;
+    if (nsub == 1) return spec_create(out, nchan, ntaps, npol, mode, nacc, window);
+    spec_ctx* p = new (std::nothrow) spec_ctx();
+    if (!p) return SPEC_ERR_NOMEM;
+    p->nsub = nsub;
+    for (int i = 0; i < nsub; i++) {
+        spec_ctx* c = nullptr;
+        int rc = spec_create(&c, nchan, ntaps, npol, mode, nacc, window);
+        if (rc) { spec_destroy(p); return rc; }
+        p->subs.push_back(c);
+    }
+    // what the parent's own entry points look at
+    p->N = nchan; p->P = npol; p->S = p->subs[0]->S; p->T = p->subs[0]->T; p->mode = mode; p->window = window; p->M = nacc;
+    *out = p;
+    return SPEC_OK;
+}
+
 extern "C" int spec_destroy(spec_t* s) {
     if (!s) return SPEC_ERR_ARG;
+    if (s->nsub > 1) {
+        for (auto c : s->subs) spec_destroy(c);
+        cudaFree(s->d_deint);
+        cudaFree(s->d_sbuf[0]); cudaFree(s->d_sbuf[1]);
+        if (s->side) cudaStreamDestroy(s->side);
+        for (int i = 0; i < 2; i++) {
+            if (s->ev_copied[i]) cudaEventDestroy(s->ev_copied[i]);
+            if (s->ev_used[i]) cudaEventDestroy(s->ev_used[i]);
+        }
+        delete s;
+        return SPEC_OK;
+    }
     cudaDeviceSynchronize();
     if (s->fused) fused_chain_quiesce();
     free_all(s);
@@ -924,6 +1044,10 @@ extern "C" int spec_destroy(spec_t* s) {
 
 extern "C" int spec_set_coeffs(spec_t* s, const float* h, size_t count) {
     if (!s || !h) return SPEC_ERR_ARG;
+    if (s->nsub > 1) {   // every sub-band runs the same filter
+        for (auto c : s->subs) { int rc = spec_set_coeffs(c, h, count); if (rc) return rc; }
+        return SPEC_OK;
+    }
     if (count != s->h_coef.size()) return SPEC_ERR_SIZE;
     CK(cudaDeviceSynchronize());
     CK(cudaMemcpy(s->d_coef, h, count * sizeof(float), cudaMemcpyHostToDevice));
@@ -939,16 +1063,120 @@ extern "C" int spec_set_coeffs(spec_t* s, const float* h, size_t count) {
 
 extern "C" int spec_get_coeffs(const spec_t* s, float* h_out, size_t count) {
     if (!s || !h_out) return SPEC_ERR_ARG;
+    if (s->nsub > 1) return spec_get_coeffs(s->subs[0], h_out, count);
     if (count != s->h_coef.size()) return SPEC_ERR_SIZE;
     memcpy(h_out, s->h_coef.data(), count * sizeof(float));
     return SPEC_OK;
 }
 
-extern "C" int spec_pending(const spec_t* s) { return s ? (int)(windows_done(s) - s->win_read) : SPEC_ERR_ARG; }
-extern "C" long spec_spectra_done(const spec_t* s) { return s ? (long)s->count : SPEC_ERR_ARG; }
+// The split fp16 DFT matrix B' of fused_producer_fft_tc: [split][k/8][col/8][col%8][k%8], k = pol*32 + 2 n1 + c,
+// col = 4 k1 + {Xre, Yre, Xim, Yim}; X[k1] = sum_n1 x[n1] exp(-2 pi i n1 k1 / 16)
+static void make_tc_matrix(std::vector<__half>& out) {
+    out.assign((size_t)kTcSplit * 64 * 64, __float2half_rn(0.f));
+    for (int col = 0; col < 64; col++)
+        for (int kk = 0; kk < 64; kk++) {
+            const int k1 = col >> 2, j = col & 3, pol = j & 1, c_out = j >> 1;
+            const int pol_in = kk >> 5, n1 = (kk & 31) >> 1, c_in = kk & 1;
+            double v = 0.0;
+            if (pol_in == pol) {
+                const double th = 2.0 * M_PI * (double)((n1 * k1) % 16) / 16.0;
+                const double cs = cos(th), sn = sin(th);
+                v = (c_out == 0) ? (c_in == 0 ? cs : sn) : (c_in == 0 ? -sn : cs);
+            }
+            if (fabs(v) < 1e-12) v = 0.0;
+            double rem = v;
+            for (int sp = 0; sp < kTcSplit; sp++) {
+                const __half h = __float2half_rn((float)rem);
+                rem -= (double)__half2float(h);
+                out[(size_t)sp * 4096 + (size_t)(kk >> 3) * 512 + (size_t)(col >> 3) * 64 + (size_t)(col & 7) * 8 + (kk & 7)] = h;
+            }
+        }
+}
+
+static int fused_failed(spec_ctx* s);
+
+// ---- CUDA-graph capture of a periodic call sequence
+extern "C" int spec_capture_begin(spec_t* s) {
+    if (!s) return SPEC_ERR_ARG;
+    if (s->nsub > 1) return SPEC_ERR_STATE;   // per-sub-band handles only
+    if (fused_failed(s)) return SPEC_ERR_CUDA;
+    if (s->capturing || s->prof) return SPEC_ERR_STATE;
+    if (windows_done(s) != s->win_read) return SPEC_ERR_STATE;   // read what is pending first
+    s->capturing = true;
+    s->cap_cur = s->cur; s->cap_fpar = s->fpar; s->cap_nhist = s->nhist;
+    s->cap_count = s->count; s->cap_win_read = s->win_read;
+    return SPEC_OK;
+}
+
+extern "C" int spec_capture_end(spec_t* s) {
+    if (!s) return SPEC_ERR_ARG;
+    if (s->nsub > 1) return SPEC_ERR_STATE;   // per-sub-band handles only
+    if (!s->capturing) return SPEC_ERR_STATE;
+    s->capturing = false;
+    const long long dcount = s->count - s->cap_count, dwin = s->win_read - s->cap_win_read;
+    // replayable only if every kernel argument baked into the graph is valid again at the end of the segment
+    const bool periodic = s->cur == s->cap_cur && s->fpar == s->cap_fpar && s->nhist == s->cap_nhist &&
+                          dcount % (s->M * (long long)s->nring) == 0 && windows_done(s) == s->win_read;
+    if (!periodic) { s->cap_dcount = 0; s->cap_dwin = 0; return SPEC_ERR_STATE; }
+    s->cap_dcount = dcount; s->cap_dwin = dwin;
+    return SPEC_OK;
+}
+
+extern "C" int spec_replayed(spec_t* s, long times) {
+    if (!s || times < 0) return SPEC_ERR_ARG;
+    if (s->nsub > 1) return SPEC_ERR_STATE;   // per-sub-band handles only
+    if (s->capturing || s->cap_dcount == 0) return SPEC_ERR_STATE;
+    s->count += s->cap_dcount * times;
+    s->win_read += s->cap_dwin * times;
+    return SPEC_OK;
+}
+
+extern "C" int spec_accumulate_host(double* h_acc, const float* h_spectrum, size_t count) {
+    if (!h_acc || !h_spectrum) return SPEC_ERR_ARG;
+    for (size_t i = 0; i < count; i++) h_acc[i] += (double)h_spectrum[i];
+    return SPEC_OK;
+}
+
+extern "C" int spec_set_option(spec_t* s, int option, int value) {
+    if (!s) return SPEC_ERR_ARG;
+    if (s->nsub > 1) {
+        for (auto c : s->subs) { int rc = spec_set_option(c, option, value); if (rc) return rc; }
+        return SPEC_OK;
+    }
+    if (option == SPEC_OPT_TENSOR_CORE_STAGE) {
+        if (value != 0 && value != 1) return SPEC_ERR_ARG;
+        // direct-FFT mode, rectangular window, dual-pol, 8192 <= nchan <= 32768 (the 16 x N2 plans of 128 threads)
+        const bool ok = s->fused && s->mode == SPEC_MODE_FFT && s->N1 == 16 && s->N2 <= 2048;
+        if (!ok) return value ? SPEC_ERR_STATE : SPEC_OK;
+        if (value && !s->d_tcB) {
+            std::vector<__half> b;
+            make_tc_matrix(b);
+            CK(cudaMalloc(&s->d_tcB, b.size() * sizeof(__half)));
+            CK(cudaMemcpy(s->d_tcB, b.data(), b.size() * sizeof(__half), cudaMemcpyHostToDevice));
+        }
+        s->tc_stage = value != 0;
+        return SPEC_OK;
+    }
+    return SPEC_ERR_ARG;
+}
+
+extern "C" int spec_pending(const spec_t* s) {
+    if (!s) return SPEC_ERR_ARG;
+    if (s->nsub > 1) return spec_pending(s->subs[0]);
+    return (int)(windows_done(s) - s->win_read);
+}
+extern "C" long spec_spectra_done(const spec_t* s) {
+    if (!s) return SPEC_ERR_ARG;
+    if (s->nsub > 1) return spec_spectra_done(s->subs[0]);
+    return (long)s->count;
+}
 
 extern "C" int spec_reset(spec_t* s) {
     if (!s) return SPEC_ERR_ARG;
+    if (s->nsub > 1) {
+        for (auto c : s->subs) { int rc = spec_reset(c); if (rc) return rc; }
+        return SPEC_OK;
+    }
     CK(cudaDeviceSynchronize());
     if (s->fused) fused_chain_quiesce();
     s->nhist = 0; s->cur = 0; s->count = 0; s->win_read = 0;
@@ -966,6 +1194,10 @@ extern "C" int spec_reset(spec_t* s) {
 
 extern "C" int spec_set_ring(spec_t* s, int nslots) {
     if (!s || nslots < 1 || nslots > 65536) return SPEC_ERR_ARG;
+    if (s->nsub > 1) {
+        for (auto c : s->subs) { int rc = spec_set_ring(c, nslots); if (rc) return rc; }
+        return SPEC_OK;
+    }
     if (s->count != 0 || s->nhist != 0) return SPEC_ERR_STATE;
     CK(cudaDeviceSynchronize());
     return alloc_ring(s, nslots);
@@ -984,8 +1216,47 @@ static int fused_failed(spec_ctx* s) {
     return 0;
 }
 
+// eight-sub-band modes: split the interleaved input into one contiguous stream per sub-band, then run every
+// sub-band's own chain on it (16 transforms per spectrum set, PAPER.md:90 step 1b) on the same stream
+static int subbands_process(spec_ctx* p, const void* d_in, size_t nsamples, cudaStream_t st) {
+    if (nsamples % (size_t)p->N) return SPEC_ERR_SIZE;
+    if (nsamples == 0) return 0;
+    if (!d_in || ((uintptr_t)d_in & 15)) return SPEC_ERR_ARG;
+    for (auto c : p->subs) {   // nothing is queued unless every sub-band accepts the call
+        if (fused_failed(c)) return SPEC_ERR_CUDA;
+        const long long total = c->nhist + (long long)(nsamples / (size_t)c->N);
+        const long long nspec = total >= c->T ? total - (c->T - 1) : 0;
+        if ((c->count + nspec) / c->M - c->win_read > c->nring - 1) return SPEC_ERR_OVERRUN;
+    }
+    const size_t wbytes = (size_t)2 * p->P;
+    if (nsamples > p->deint_cap) {
+        cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cap) == cudaSuccess && cap != cudaStreamCaptureStatusNone) return SPEC_ERR_STATE;
+        CK(cudaDeviceSynchronize());
+        uint8_t* nb = nullptr;
+        CK(cudaMalloc(&nb, nsamples * wbytes * p->nsub));
+        cudaFree(p->d_deint);
+        p->d_deint = nb;
+        p->deint_cap = nsamples;
+    }
+    const int gx = cdiv((long long)nsamples, 256);
+    if (p->P == 2)
+        k_deinterleave<uint32_t><<<gx, 256, 0, st>>>((const uint32_t*)d_in, (uint32_t*)p->d_deint, nsamples, p->nsub, p->deint_cap);
+    else
+        k_deinterleave<uint16_t><<<gx, 256, 0, st>>>((const uint16_t*)d_in, (uint16_t*)p->d_deint, nsamples, p->nsub, p->deint_cap);
+    CK(cudaGetLastError());
+    int completed = 0;
+    for (int i = 0; i < p->nsub; i++) {
+        const int rc = spec_process(p->subs[i], p->d_deint + (size_t)i * p->deint_cap * wbytes, nsamples, st);
+        if (rc < 0) return rc;
+        completed = rc;
+    }
+    return completed;
+}
+
 extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* cuda_stream) {
     if (!s) return SPEC_ERR_ARG;
+    if (s->nsub > 1) return subbands_process(s, d_in, nsamples, (cudaStream_t)cuda_stream);
     if (fused_failed(s)) return SPEC_ERR_CUDA;
     if (nsamples % (size_t)s->N) return SPEC_ERR_SIZE;
     if (nsamples == 0) return 0;
@@ -1048,6 +1319,14 @@ extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* 
 
 extern "C" int spec_read_accum(spec_t* s, float* dst, int dst_is_device, void* cuda_stream) {
     if (!s || !dst) return SPEC_ERR_ARG;
+    if (s->nsub > 1) {   // [nsub][S][nchan]
+        int got = 0;
+        for (int i = 0; i < s->nsub; i++) {
+            got = spec_read_accum(s->subs[i], dst + (size_t)i * s->S * s->N, dst_is_device, cuda_stream);
+            if (got <= 0) return got;
+        }
+        return got;
+    }
     if (fused_failed(s)) return SPEC_ERR_CUDA;
     if (windows_done(s) - s->win_read <= 0) return 0;
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -1068,6 +1347,16 @@ extern "C" int spec_read_accum(spec_t* s, float* dst, int dst_is_device, void* c
 
 extern "C" int spec_read_accum_batch(spec_t* s, float* d_dst, int max_count, void* cuda_stream) {
     if (!s || !d_dst || max_count < 0) return SPEC_ERR_ARG;
+    if (s->nsub > 1) {   // [count][nsub][S][nchan]
+        int n = spec_pending(s);
+        if (n > max_count) n = max_count;
+        for (int c = 0; c < n; c++)
+            for (int i = 0; i < s->nsub; i++) {
+                const int rc = spec_read_accum(s->subs[i], d_dst + ((size_t)c * s->nsub + i) * s->S * s->N, 1, cuda_stream);
+                if (rc < 0) return rc;
+            }
+        return n;
+    }
     if (fused_failed(s)) return SPEC_ERR_CUDA;
     long long n = windows_done(s) - s->win_read;
     if (n > max_count) n = max_count;
@@ -1088,7 +1377,7 @@ extern "C" int spec_stream_host(spec_t* s, const void* h_pinned, size_t nsamples
     if (!s || (!h_pinned && nsamples)) return SPEC_ERR_ARG;
     if (chunk_samples == 0 || chunk_samples % (size_t)s->N || nsamples % (size_t)s->N) return SPEC_ERR_SIZE;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t bps = (size_t)2 * s->P;
+    const size_t bps = (size_t)2 * s->P * s->nsub;
     const size_t cbytes = chunk_samples * bps;
     if (!s->side) {
         CK(cudaStreamCreateWithFlags(&s->side, cudaStreamNonBlocking));
@@ -1170,6 +1459,7 @@ extern "C" int spec_debug_unpack(const void* d_bytes, size_t nbytes, int npol, f
 // window code: a DUMP instantiation of the same kernel template) and writes what it hands to the first butterfly.
 extern "C" int spec_debug_fir(spec_t* s, const void* d_blocks, int nspec, float* d_out, void* cuda_stream) {
     if (!s || !d_blocks || !d_out || nspec < 1 || ((uintptr_t)d_blocks & 15)) return SPEC_ERR_ARG;
+    if (s->nsub > 1) return SPEC_ERR_STATE;   // per-sub-band handles only
     if (fused_failed(s)) return SPEC_ERR_CUDA;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     InputView view{nullptr, (const uint8_t*)d_blocks, 0};
@@ -1203,6 +1493,12 @@ extern "C" int spec_debug_hog(int ms, size_t smem_bytes, void* cuda_stream) {
 
 extern "C" int spec_plan_info(const spec_t* s, int* n1, int* n2, char* desc, size_t desc_len) {
     if (!s) return SPEC_ERR_ARG;
+    if (s->nsub > 1) {
+        char sub[400] = "";
+        int rc = spec_plan_info(s->subs[0], n1, n2, sub, sizeof(sub));
+        if (desc && desc_len) snprintf(desc, desc_len, "%d sub-bands: k_deinterleave, then per sub-band %s", s->nsub, sub);
+        return rc;
+    }
     if (n1) *n1 = s->N1;
     if (n2) *n2 = s->N2;
     if (desc && desc_len) {
@@ -1228,6 +1524,10 @@ extern "C" int spec_plan_info(const spec_t* s, int* n1, int* n2, char* desc, siz
 
 extern "C" int spec_profile(spec_t* s, int enable) {
     if (!s) return SPEC_ERR_ARG;
+    if (s->nsub > 1) {
+        for (auto c : s->subs) spec_profile(c, enable);
+        return SPEC_OK;
+    }
     prof_fold(s);
     s->prof = enable != 0;
     for (int i = 0; i < 4; i++) { s->prof_ms[i] = 0; s->prof_n[i] = 0; }
@@ -1236,6 +1536,15 @@ extern "C" int spec_profile(spec_t* s, int enable) {
 
 extern "C" int spec_profile_read(spec_t* s, double ms[4], long launches[4]) {
     if (!s || !ms || !launches) return SPEC_ERR_ARG;
+    if (s->nsub > 1) {
+        for (int i = 0; i < 4; i++) { ms[i] = 0; launches[i] = 0; }
+        for (auto c : s->subs) {
+            double m[4]; long l[4];
+            spec_profile_read(c, m, l);
+            for (int i = 0; i < 4; i++) { ms[i] += m[i]; launches[i] += l[i]; }
+        }
+        return SPEC_OK;
+    }
     prof_fold(s);
     for (int i = 0; i < 4; i++) { ms[i] = s->prof_ms[i]; launches[i] = s->prof_n[i]; }
     return SPEC_OK;

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libspec.so")
 
 MODE_PFB, MODE_FFT = 0, 1
 WINDOW_RECT, WINDOW_HANN = 0, 1
+OPT_TENSOR_CORE_STAGE = 1
 OK, ERR_ARG, ERR_STATE, ERR_SIZE, ERR_OVERRUN, ERR_CUDA, ERR_NOMEM = 0, -1, -2, -3, -4, -5, -6
 
 # every symbol include/spec.h declares (tests check the library exports all of them)
@@ -25,7 +26,8 @@ SYMBOLS = [
     "spec_pending", "spec_spectra_done", "spec_reset", "spec_set_ring", "spec_get_coeffs",
     "spec_stream_host", "spec_measure_fp32_peak", "spec_debug_unpack", "spec_debug_fir",
     "spec_strerror", "spec_last_error", "spec_profile", "spec_profile_read", "spec_read_accum_batch",
-    "spec_plan_info", "spec_debug_hog",
+    "spec_plan_info", "spec_debug_hog", "spec_set_option", "spec_capture_begin", "spec_capture_end", "spec_replayed",
+    "spec_accumulate_host", "spec_create_subbands",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -36,6 +38,7 @@ if not os.path.exists(LIB_PATH):
 _lib = C.CDLL(LIB_PATH)
 _vp, _sz, _fp = C.c_void_p, C.c_size_t, C.POINTER(C.c_float)
 _lib.spec_create.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_int, C.c_long, C.c_int]
+_lib.spec_create_subbands.argtypes = [C.POINTER(_vp), C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.c_long, C.c_int]
 _lib.spec_set_coeffs.argtypes = [_vp, _fp, _sz]
 _lib.spec_process.argtypes = [_vp, _vp, _sz, _vp]
 _lib.spec_read_accum.argtypes = [_vp, _vp, C.c_int, _vp]
@@ -52,6 +55,11 @@ _lib.spec_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), _vp]
 _lib.spec_debug_unpack.argtypes = [_vp, _sz, C.c_int, _vp, _vp]
 _lib.spec_debug_fir.argtypes = [_vp, _vp, C.c_int, _vp, _vp]
 _lib.spec_debug_hog.argtypes = [C.c_int, _sz, _vp]
+_lib.spec_set_option.argtypes = [_vp, C.c_int, C.c_int]
+_lib.spec_capture_begin.argtypes = [_vp]
+_lib.spec_capture_end.argtypes = [_vp]
+_lib.spec_replayed.argtypes = [_vp, C.c_long]
+_lib.spec_accumulate_host.argtypes = [C.POINTER(C.c_double), _fp, _sz]
 _lib.spec_plan_info.argtypes = [_vp, C.POINTER(C.c_int), C.POINTER(C.c_int), C.c_char_p, _sz]
 _lib.spec_profile.argtypes = [_vp, C.c_int]
 _lib.spec_profile_read.argtypes = [_vp, C.POINTER(C.c_double), C.POINTER(C.c_long)]
@@ -92,13 +100,26 @@ def debug_hog(ms, smem_bytes, stream=0):
     _check(_lib.spec_debug_hog(ms, smem_bytes, stream), "spec_debug_hog")
 
 
+def accumulate_host(h_acc, h_spectrum):
+    """h_acc (float64, C-contiguous) += h_spectrum (float32), in the library (the CPU thread)."""
+    assert h_acc.dtype == np.float64 and h_spectrum.dtype == np.float32 and h_acc.size == h_spectrum.size
+    assert h_acc.flags.c_contiguous and h_spectrum.flags.c_contiguous
+    _check(_lib.spec_accumulate_host(h_acc.ctypes.data_as(C.POINTER(C.c_double)), h_spectrum.ctypes.data_as(_fp),
+                                     h_acc.size), "spec_accumulate_host")
+
+
 class Spec:
     """Thin handle around spec_t*.  Pointers are integers (device or host addresses)."""
 
-    def __init__(self, nchan, ntaps, npol, mode, nacc, window=WINDOW_HANN):
+    def __init__(self, nchan, ntaps, npol, mode, nacc, window=WINDOW_HANN, nsub=1):
         h = _vp()
-        _check(_lib.spec_create(C.byref(h), nchan, ntaps, npol, mode, nacc, window), "spec_create")
+        if nsub == 1:
+            _check(_lib.spec_create(C.byref(h), nchan, ntaps, npol, mode, nacc, window), "spec_create")
+        else:
+            _check(_lib.spec_create_subbands(C.byref(h), nsub, nchan, ntaps, npol, mode, nacc, window),
+                   "spec_create_subbands")
         self._h = h
+        self.nsub = nsub
         self.nchan, self.npol, self.mode, self.nacc = nchan, npol, mode, nacc
         self.ntaps = 1 if mode == MODE_FFT else ntaps
         self.nstokes = 4 if npol == 2 else 1
@@ -124,7 +145,8 @@ class Spec:
         return _check(_lib.spec_read_accum_batch(self._h, d_dst_ptr, max_count, stream), "spec_read_accum_batch")
 
     def read_accum_host(self, stream=0):
-        out = np.empty((self.nstokes, self.nchan), dtype=np.float32)
+        shape = (self.nstokes, self.nchan) if self.nsub == 1 else (self.nsub, self.nstokes, self.nchan)
+        out = np.empty(shape, dtype=np.float32)
         rc = _check(_lib.spec_read_accum(self._h, out.ctypes.data, 0, stream), "spec_read_accum")
         return out if rc == 1 else None
 
@@ -140,6 +162,18 @@ class Spec:
 
     def reset(self):
         _check(_lib.spec_reset(self._h), "spec_reset")
+
+    def set_option(self, option, value):
+        _check(_lib.spec_set_option(self._h, option, value), "spec_set_option")
+
+    def capture_begin(self):
+        _check(_lib.spec_capture_begin(self._h), "spec_capture_begin")
+
+    def capture_end(self):
+        _check(_lib.spec_capture_end(self._h), "spec_capture_end")
+
+    def replayed(self, times):
+        _check(_lib.spec_replayed(self._h, times), "spec_replayed")
 
     def set_ring(self, nslots):
         _check(_lib.spec_set_ring(self._h, nslots), "spec_set_ring")

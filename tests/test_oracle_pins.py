@@ -418,3 +418,59 @@ def test_generator_is_split_invariant():
     a = synth.config_stream(1, 0, 3 * (1 << 20) + 17)
     b = np.concatenate([synth.config_stream(1, 0, (1 << 20) - 5), synth.config_stream(1, (1 << 20) - 5, 2 * (1 << 20) + 22)])
     np.testing.assert_array_equal(a, b)
+
+
+# ---------------------------------------------------------------- eight-sub-band modes
+
+def test_subband_oracle_places_each_sub_band_in_its_own_output():
+    """Reading R26 (sub-bands interleaved per time sample, sub-band 0 first): a tone fed to ONE sub-band shows up
+    in that sub-band's output only, at its own channel; the others hold noise-free zeros."""
+    N, nsub, M = 64, 8, 4
+    j = np.arange(M * N)
+    for hot, chan in ((0, 5), (3, 17), (7, 60)):
+        raw = np.zeros((M * N, nsub, 4), dtype=np.int8)
+        z = 50.0 * np.exp(2j * np.pi * chan * j / N)
+        raw[:, hot, 0] = np.rint(z.real)
+        raw[:, hot, 1] = np.rint(z.imag)
+        o = oracle.OracleSub(nsub, N, 1, 2, oracle.MODE_FFT, M, oracle.WINDOW_RECT)
+        assert o.process(raw) == 1
+        out = o.read_accum()
+        o.close()
+        assert out.shape == (nsub, 4, N)
+        for s in range(nsub):
+            if s == hot:
+                assert np.argmax(out[s, 0]) == chan
+                assert out[s, 0, chan] > 0.99 * out[s, 0].sum()
+            else:
+                assert np.all(out[s] == 0)
+
+
+def test_subband_oracle_equals_the_single_band_oracle_on_every_sub_band():
+    """Each sub-band is the single-sub-band chain on its own samples: identical streams in all sub-bands give
+    outputs bit-identical to the plain oracle's, and permuting the sub-bands of the input permutes the outputs."""
+    N, T, nsub, M = 128, 4, 8, 3
+    rng = np.random.default_rng(7)
+    base = rng.integers(-128, 128, size=((2 * M + T - 1) * N, 4), dtype=np.int8)
+    one = oracle.Oracle(N, T, 2, oracle.MODE_PFB, M)
+    one.process(base)
+    ref = [one.read_accum(), one.read_accum()]
+    one.close()
+    raw = np.repeat(base[:, None, :], nsub, axis=1)
+    o = oracle.OracleSub(nsub, N, T, 2, oracle.MODE_PFB, M)
+    assert o.process(raw) == 2
+    for w in range(2):
+        out = o.read_accum()
+        for s in range(nsub):
+            assert np.array_equal(out[s], ref[w])
+    o.close()
+    # different data per sub-band; a permutation of the sub-bands permutes the outputs
+    data = rng.integers(-128, 128, size=((M + T - 1) * N, nsub, 4), dtype=np.int8)
+    perm = rng.permutation(nsub)
+    a = oracle.OracleSub(nsub, N, T, 2, oracle.MODE_PFB, M)
+    b = oracle.OracleSub(nsub, N, T, 2, oracle.MODE_PFB, M)
+    a.process(data)
+    b.process(data[:, perm, :])
+    oa, ob = a.read_accum(), b.read_accum()
+    a.close(); b.close()
+    assert np.array_equal(ob, oa[perm])
+    assert not np.array_equal(oa[0], oa[1])

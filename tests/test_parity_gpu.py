@@ -62,7 +62,7 @@ FRONT_PFB = [(64, 4, 1, "k_engine"), (64, 4, 2, "k_engine"), (1024, 8, 1, "k_eng
              (1024, 8, 2, "k_fused"), (2048, 8, 2, "k_fused"), (4096, 8, 2, "k_fused"), (8192, 8, 2, "k_fused"),
              (16384, 8, 2, "k_fused"), (32768, 8, 2, "k_fused"), (65536, 8, 2, "k_fused"),
              (8192, 8, 1, "k_passA_pfb16"), (8192, 4, 2, "k_engine pass A"), (131072, 8, 1, "k_fir8"),
-             (131072, 8, 2, None), (524288, 8, 2, None)]
+             (131072, 8, 2, "k_fused"), (262144, 8, 2, "k_fused"), (524288, 8, 2, "k_fused")]
 
 
 @pytest.mark.parametrize("nchan,ntaps,npol,kernel", FRONT_PFB)
@@ -86,7 +86,7 @@ def test_indexing_bit_exact_with_single_tap_coefficients(nchan, ntaps, npol, ker
 
 
 FRONT_FFT = [(256, 2, "k_engine"), (4096, 2, "k_engine"), (4096, 1, "k_engine"), (8192, 2, "k_fused"),
-             (32768, 2, "k_fused"), (65536, 2, "k_fused"), (16384, 1, "k_engine pass A"), (262144, 2, None)]
+             (32768, 2, "k_fused"), (65536, 2, "k_fused"), (16384, 1, "k_engine pass A"), (131072, 2, "k_fused"), (262144, 2, "k_fused"), (524288, 2, "k_fused")]
 
 
 @pytest.mark.parametrize("nchan,npol,kernel", FRONT_FFT)
@@ -187,6 +187,24 @@ def test_parity_fused_kernel_ring_wraps(nchan, mode, nspec, M):
     assert len(g) == len(r) == nspec // M
     for a, b in zip(g, r):
         compare(a, b, f"fused ring N={nchan} mode={mode}")
+
+
+@pytest.mark.parametrize("nchan,mode,nspec,M", [(131072, PFB, 61, 25), (131072, FFT, 50, 16), (262144, PFB, 37, 11),
+                                                (262144, FFT, 30, 30), (524288, PFB, 21, 16), (524288, FFT, 19, 6)])
+def test_parity_fused_kernel_largest_sizes_ring_wraps(nchan, mode, nspec, M):
+    """N >= 131072: the persistent kernel with N1 = 32, 64, 128 column transforms (two-stage, in place in shared
+    memory) and 4096-point rows; more spectra than its small L2-resident ring holds, two calls, ragged last group."""
+    T = 8 if mode == PFB else 1
+    nblk = nspec + T - 1
+    raw = synth.dual_pol_stream(500 + nchan // 65536 + mode, nblk * nchan, [synth.F_CFG1])
+    w = 1 if mode == PFB else 0
+    g, gd = gpu_run(raw, nchan, T, 2, mode, M, window=w, splits=[nchan * (nblk - 9), nchan * 9], ring=16)
+    r, rd = oracle_run(raw, nchan, T, 2, mode, M, window=w)
+    assert gd == rd == nspec
+    assert len(g) == len(r) == nspec // M
+    for a, b in zip(g, r):
+        compare(a, b, f"fused large N={nchan} mode={mode}")
+        check_stokes_invariants(a)
 
 
 def test_two_handles_on_two_streams_share_the_gpu():
@@ -437,6 +455,200 @@ def test_sweep_longest_accumulation_2e21_spectra(sweep_refs):
     s.close()
     w = compare(got, reps * np.asarray(outs_ref[0]), "N=1024 FFT M=2^21")
     assert w["rel_l2"] < 3e-5
+
+
+# ---------------------------------------------------------------- NEXT-2: first DFT factor on the tensor cores
+
+@pytest.mark.parametrize("nchan", [8192, 16384, 32768])
+@pytest.mark.parametrize("stream", ["random_bytes", "config1"])
+def test_tensor_core_first_stage_parity(nchan, stream):
+    """spec_set_option(SPEC_OPT_TENSOR_CORE_STAGE): the 16-point column DFT of the direct-FFT plans as a tcgen05.mma
+    contraction (fp16 samples, exact; DFT matrix split into two fp16 terms; fp32 accumulation in tensor memory).
+    Same tolerances as every other path (north_star: "only if the stated tolerance still holds"); full-range bytes
+    exercise -128 and the largest sums, the config-1 stream a ring that wraps."""
+    torch, sp = _torch(), _sp()
+    M = 37
+    nspec = 3 * M + 5 if stream == "config1" else M + 3
+    raw = (synth.dual_pol_stream(1500 + nchan // 1024, nspec * nchan, [synth.F_CFG1]) if stream == "config1"
+           else synth.random_bytes(1600 + nchan // 1024, nspec * nchan, 2))
+    r, rd = oracle_run(raw, nchan, 1, 2, FFT, M, window=0)
+    d = torch.from_numpy(raw.reshape(-1)).cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    errs = {}
+    for tc in (0, 1):
+        s = sp.Spec(nchan, 1, 2, FFT, M, 0)
+        s.set_option(sp.OPT_TENSOR_CORE_STAGE, tc)
+        s.process(d.data_ptr(), (nspec - 7) * nchan, st)
+        s.process(d.data_ptr() + (nspec - 7) * nchan * 4, 7 * nchan, st)
+        assert s.spectra_done() == rd
+        outs = []
+        while s.pending():
+            outs.append(s.read_accum_host(st))
+        s.close()
+        assert len(outs) == len(r)
+        worst = 0.0
+        for a, b in zip(outs, r):
+            worst = max(worst, compare(a, b, f"tc={tc} N={nchan} {stream}")["rel_l2"])
+            check_stokes_invariants(a)
+        errs[tc] = worst
+    print(f"N={nchan} {stream}: rel L2 fp32 stage {errs[0]:.2e}, tensor-core stage {errs[1]:.2e}")
+    assert errs[1] < 2e-5
+
+
+def test_tensor_core_option_rejected_where_the_plan_has_no_such_stage():
+    sp = _sp()
+    for args in ((32768, 8, 2, PFB, 4, 1), (4096, 1, 2, FFT, 4, 0), (65536, 1, 2, FFT, 4, 0), (8192, 1, 1, FFT, 4, 0)):
+        s = sp.Spec(*args)
+        with pytest.raises(sp.SpecError) as e:
+            s.set_option(sp.OPT_TENSOR_CORE_STAGE, 1)
+        assert e.value.code == sp.ERR_STATE
+        s.set_option(sp.OPT_TENSOR_CORE_STAGE, 0)
+        s.close()
+
+
+# ---------------------------------------------------------------- NEXT-4: packet-sized calls replayed as a CUDA graph
+
+@pytest.mark.parametrize("nchan,mode,ntaps", [(1024, PFB, 8), (256, PFB, 4), (8192, FFT, 1)])
+def test_cuda_graph_replay_of_packet_sized_calls(nchan, mode, ntaps):
+    """A periodic segment of 18 small spec_process calls (8 blocks each) and its read-outs is captured once and
+    replayed on fresh input; the filter history and the accumulation windows carry on across replays on the device.
+    The host then sums the read-outs in double precision (the CPU thread)."""
+    torch, sp = _torch(), _sp()
+    T = ntaps if mode == PFB else 1
+    M, bpc, ncalls, nrep = 16, 8, 18, 4
+    seg_blocks = bpc * ncalls                      # 144 spectra per segment = 9 windows = the ring's period
+    raw = synth.dual_pol_stream(1700 + nchan, ((T - 1) + nrep * seg_blocks) * nchan, [synth.F_CFG1])
+    w = 1 if mode == PFB else 0
+    r, rd = oracle_run(raw, nchan, T, 2, mode, M, window=w)
+    assert len(r) == nrep * 9
+    s = sp.Spec(nchan, T, 2, mode, M, w)
+    st0 = torch.cuda.current_stream().cuda_stream
+    d_all = torch.from_numpy(raw.reshape(-1)).cuda()
+    if T > 1:
+        s.process(d_all.data_ptr(), (T - 1) * nchan, st0)          # fill the history outside the graph
+    seg_bytes = seg_blocks * nchan * 4
+    d_seg = torch.empty(seg_bytes, dtype=torch.int8, device="cuda")
+    d_out = torch.zeros((9, 4, nchan), dtype=torch.float32, device="cuda")
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        st = torch.cuda.current_stream().cuda_stream
+        s.capture_begin()
+        got = 0
+        for c in range(ncalls):
+            s.process(d_seg.data_ptr() + c * bpc * nchan * 4, bpc * nchan, st)
+            if c % 6 == 5:
+                got += s.read_accum_batch_device(d_out.data_ptr() + got * 4 * nchan * 4, 8, st)
+        assert got == 9
+        s.capture_end()
+    outs = []
+    hist = (T - 1) * nchan * 4
+    for rep in range(nrep):
+        d_seg.copy_(d_all[hist + rep * seg_bytes: hist + (rep + 1) * seg_bytes])
+        g.replay()
+        outs += list(d_out.cpu().numpy())
+    s.replayed(nrep - 1)
+    assert s.spectra_done() == rd and s.pending() == 0
+    s.close()
+    total = np.zeros((4, nchan), dtype=np.float64)
+    for a, b in zip(outs, r):
+        compare(a, b, f"graph replay N={nchan}")
+        sp.accumulate_host(total, np.ascontiguousarray(a))
+    compare(total, np.sum(np.asarray(r), axis=0), "host-side long accumulation")
+
+
+def test_cuda_graph_capture_rejects_a_segment_that_is_not_periodic():
+    torch, sp = _torch(), _sp()
+    N = 1024
+    s = sp.Spec(N, 8, 2, PFB, 16)
+    d = torch.zeros(64 * N * 4, dtype=torch.int8, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    s.process(d.data_ptr(), 7 * N, st)
+    torch.cuda.synchronize()
+    s.capture_begin()                     # (no stream capture needed to exercise the bookkeeping)
+    for c in range(5):                    # 5 calls: the history buffers and ring parities do not line up again
+        s.process(d.data_ptr(), 8 * N, st)
+    while s.pending():
+        s.read_accum_host(st)
+    with pytest.raises(sp.SpecError) as e:
+        s.capture_end()
+    assert e.value.code == sp.ERR_STATE
+    s.close()
+
+
+# ---------------------------------------------------------------- NEXT-3: eight-sub-band modes
+
+@pytest.mark.parametrize("nchan,mode,ntaps,nsub,npol", [(4096, PFB, 8, 8, 2), (16384, PFB, 8, 8, 2), (65536, PFB, 8, 8, 2),
+                                                        (4096, FFT, 1, 8, 2), (8192, FFT, 1, 8, 2), (1024, PFB, 4, 3, 1)])
+def test_parity_sub_band_modes(nchan, mode, ntaps, nsub, npol):
+    """eight sub-bands x two polarisations = 16 transforms per spectrum set, channel counts of
+    Table 1's third block; the input interleaves the sub-bands per time sample (reading R26).  Different data in
+    every sub-band (each gets its own tone), two calls, windows that straddle them."""
+    import oracle
+    torch, sp = _torch(), _sp()
+    T = ntaps if mode == PFB else 1
+    M = 5
+    nblk = 2 * M + (T - 1) + 3
+    ns = nblk * nchan
+    rng = np.random.default_rng(nchan + nsub)
+    raw = rng.integers(-40, 41, size=(ns, nsub, 2 * npol)).astype(np.float64)
+    j = np.arange(ns)
+    for s in range(nsub):   # a tone of its own per sub-band, in polarisation 0
+        z = 30.0 * np.exp(2j * np.pi * ((37 + 11 * s) % nchan) * j / nchan)
+        raw[:, s, 0] += z.real
+        raw[:, s, 1] += z.imag
+    raw = np.clip(np.rint(raw), -128, 127).astype(np.int8)
+    w = 1 if mode == PFB else 0
+    o = oracle.OracleSub(nsub, nchan, T, npol, mode, M, w)
+    o.process(raw)
+    ref = []
+    while o.pending():
+        ref.append(o.read_accum())
+    rd = o.spectra_done()
+    o.close()
+    s_ = sp.Spec(nchan, T, npol, mode, M, w, nsub=nsub)
+    n1, n2, desc = s_.plan_info()
+    assert f"{nsub} sub-bands" in desc
+    d = torch.from_numpy(raw.reshape(-1)).cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    bps = nsub * 2 * npol
+    first = (nblk - 4) * nchan
+    got = []
+    done = s_.process(d.data_ptr(), first, st)
+    done += s_.process(d.data_ptr() + first * bps, ns - first, st)
+    assert done == len(ref) == 2 and s_.spectra_done() == rd
+    while s_.pending():
+        got.append(s_.read_accum_host(st))
+    s_.close()
+    for a, b in zip(got, ref):
+        assert a.shape == b.shape == (nsub, 4 if npol == 2 else 1, nchan)
+        for s in range(nsub):
+            compare(a[s], b[s], f"sub-band {s} of {nsub}, N={nchan} mode={mode}")
+            assert np.argmax(a[s][0]) == (37 + 11 * s) % nchan
+
+
+def test_sub_band_stream_host_and_batch_read():
+    torch, sp = _torch(), _sp()
+    import oracle
+    N, T, M, nsub = 4096, 8, 4, 8
+    nblk = 3 * M + T - 1
+    rng = np.random.default_rng(99)
+    raw = rng.integers(-128, 128, size=(nblk * N, nsub, 4), dtype=np.int8)
+    o = oracle.OracleSub(nsub, N, T, 2, oracle.MODE_PFB, M)
+    o.process(raw)
+    ref = [o.read_accum() for _ in range(3)]
+    o.close()
+    hp = torch.from_numpy(raw.reshape(-1)).pin_memory()
+    st = torch.cuda.current_stream().cuda_stream
+    s = sp.Spec(N, T, 2, PFB, M, nsub=nsub)
+    assert s.stream_host(hp.data_ptr(), nblk * N, 5 * N, st) == 3
+    out = torch.zeros((3, nsub, 4, N), dtype=torch.float32, device="cuda")
+    assert s.read_accum_batch_device(out.data_ptr(), 8, st) == 3
+    got = out.cpu().numpy()
+    s.close()
+    for c in range(3):
+        for k in range(nsub):
+            compare(got[c, k], ref[c][k], f"sub-band batch read {c}/{k}")
 
 
 # ---------------------------------------------------------------- BASELINE.json configs
