@@ -515,7 +515,7 @@ def main():
     p.add_argument("--nacc", type=int, default=0)
     p.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     p.add_argument("--tensor-core-stage", action="store_true",
-                   help="direct-FFT mode, 8192 <= N <= 32768: first DFT factor via tcgen05.mma (spec_set_option)")
+                   help="direct-FFT mode, N = 16384 or 32768: first DFT factor via tcgen05.mma (spec_set_option)")
     p.add_argument("--sweep", action="store_true", help="configs[4]: all 20 points, resident and streamed")
     p.add_argument("--sweep-log2", type=int, default=31, help="log2 of the time samples per sweep point")
     p.add_argument("--sweep-reps", type=int, default=3)

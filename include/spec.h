@@ -140,7 +140,7 @@ int spec_replayed(spec_t* s, long times);
 int spec_accumulate_host(double* h_acc, const float* h_spectrum, size_t count);
 
 /* Plan options.  SPEC_OPT_TENSOR_CORE_STAGE (value 0 / 1): in direct-FFT mode with the rectangular window
- * (dual-pol, 8192 <= nchan <= 32768) run the first 16-point DFT factor of the four-step transform on the tensor
+ * (dual-pol, nchan 16384 or 32768) run the first 16-point DFT factor of the four-step transform on the tensor
  * cores (tcgen05.mma, fp16 operands: the int8 samples are exact, the DFT matrix is split into two fp16 terms,
  * fp32 accumulation) instead of fp32 butterflies.  Off by default; DESIGN.md section 7
  * records the measured speed and error of both.  SPEC_ERR_STATE if the handle's plan has no such stage. */

@@ -89,7 +89,7 @@ struct FrontRaw {
         return (blk < view.nhist) ? view.hist + (size_t)blk * N * (2 * P)
                                   : view.in + (size_t)(blk - view.nhist) * N * (2 * P);
     }
-    __device__ __forceinline__ cpx decode(const void* x, int e) const {
+    __device__ __forceinline__ cpx decode(const void* x, int e, int = 0) const {
         const uint32_t w = (P == 2) ? ((const uint32_t*)x)[e] : (uint32_t)((const uint16_t*)x)[e];
         cpx v = unpack_cpx<P>(w);
         if (WIN) {
@@ -132,6 +132,45 @@ struct FrontRaw {
     }
 };
 
+// Direct-FFT front end for N = 2 L with NO intermediate: slot variant r (0 / 1) computes the even / odd channels of the
+// N-point transform as ONE L-point transform of  x[n] + x[n+L]  /  (x[n] - x[n+L]) W_N^n  (the first radix-2
+// decimation-in-frequency layer), each from the whole raw block.  The unpack is done twice, in exchange
+// the 16 B per sample four-step intermediate and its cross-SM hand-over disappear (N = 8192: one k_engine launch).
+template <int WIN>
+struct FrontRawR2 {
+    InputView view;
+    const float2* twN;   // W_N^e
+    const float* h;      // WIN: window over N
+    int N, L;            // N = 2 L
+    long long m0;
+    int stride = 1;      // (dump_put)
+    static constexpr bool kBulk = true;
+    static constexpr int kElemBytes = 8;   // element e of the staged block = samples e and e + L
+    __device__ __forceinline__ const void* src(long long job, int) const {
+        const long long blk = m0 + job;
+        return (blk < view.nhist) ? view.hist + (size_t)blk * N * 4 : view.in + (size_t)(blk - view.nhist) * N * 4;
+    }
+    __device__ __forceinline__ int off(int variant) const { return variant; }
+    __device__ __forceinline__ cpx decode(const void* x, int e, int r) const {
+        cpx a = unpack_cpx<2>(((const uint32_t*)x)[e]), b = unpack_cpx<2>(((const uint32_t*)x)[e + L]);
+        if (WIN) {
+            const u64 ca = bc(__ldg(h + e)), cb = bc(__ldg(h + e + L));
+            a = {mul2(a.re, ca), mul2(a.im, ca)};
+            b = {mul2(b.re, cb), mul2(b.im, cb)};
+        }
+        if (r == 0) return cadd(a, b);
+        const float2 w = __ldg(twN + e);
+        return cmul(csub(a, b), w.x, w.y);
+    }
+    __device__ __forceinline__ cpx load(long long job, int e, int r) const { return decode(src(job, r), e, r); }
+    // test hook: what this front end hands to the L-point transform, [job][r][e]: r = 0 the sums x[e] + x[e+L]
+    // (exact integers), r = 1 the twiddled differences
+    __device__ __forceinline__ void dump_put(float* dump, long long job, int e, int r, cpx v) const {
+        const float4 z = cpx_to_f4(v);
+        ((float4*)dump)[(size_t)job * N + (size_t)r * L + e] = make_float4(z.x, z.z, z.y, z.w);
+    }
+};
+
 // front end for `pass B`: row `slot_id` of the intermediate Z[m][row][n2] (float4 = Xre,Yre,Xim,Yim)
 struct FrontZ {
     const float4* Z;
@@ -141,7 +180,7 @@ struct FrontZ {
     __device__ __forceinline__ const void* src(long long m, int row) const {
         return Z + (size_t)m * N + (size_t)row * N2;
     }
-    __device__ __forceinline__ cpx decode(const void* x, int e) const { return f4_to_cpx(((const float4*)x)[e]); }
+    __device__ __forceinline__ cpx decode(const void* x, int e, int = 0) const { return f4_to_cpx(((const float4*)x)[e]); }
     __device__ __forceinline__ int off(int slot_id) const { return slot_id; }
     __device__ __forceinline__ void dump_put(float*, long long, int, int, cpx) const {}
     __device__ __forceinline__ cpx load(long long m, int e, int row) const {
@@ -158,13 +197,22 @@ struct FrontY {
     static constexpr bool kBulk = false;
     static constexpr int kElemBytes = 16;
     __device__ __forceinline__ const void* src(long long, int) const { return nullptr; }
-    __device__ __forceinline__ cpx decode(const void*, int) const { return {0ull, 0ull}; }
+    __device__ __forceinline__ cpx decode(const void*, int, int = 0) const { return {0ull, 0ull}; }
     __device__ __forceinline__ int off(int slot_id) const { return slot_id; }
     __device__ __forceinline__ void dump_put(float*, long long, int, int, cpx) const {}
     __device__ __forceinline__ cpx load(long long m, int e, int off_) const {
         return f4_to_cpx(__ldcg(Y + (size_t)m * N + (size_t)e * stride + off_));
     }
 };
+
+// accumulator update without a return value: one vector reduction at the L2 (RED.E.ADD.F32x4), nothing comes back
+// to the SM (atomicAdd(float4*) compiles to ATOMG, whose result the thread then waits for)
+__device__ __forceinline__ void red_add_f4(float4* p, float a, float b, float c, float d) {
+    asm volatile("red.relaxed.gpu.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+__device__ __forceinline__ void red_add_f1(float* p, float a) {
+    asm volatile("red.relaxed.gpu.global.add.f32 [%0], %1;" ::"l"(p), "f"(a) : "memory");
+}
 
 // ---- sinks
 // The last engine stage hands each sink the 16 outputs of one radix-16 butterfly at once:
@@ -211,8 +259,8 @@ struct SinkStokes {
         for (int q = 0; q < 16; q++) {
             float xx, yy;
             upk(s.pw[q], xx, yy);
-            if (P == 2) atomicAdd((float4*)acc + pos + q, make_float4(xx, yy, s.cr[q], s.ci[q]));
-            else atomicAdd(acc + pos + q, xx);
+            if (P == 2) red_add_f4((float4*)acc + pos + q, xx, yy, s.cr[q], s.ci[q]);
+            else red_add_f1(acc + pos + q, xx);
         }
     }
 };
@@ -351,7 +399,7 @@ struct SinkStokesTmem {
             tmem_wait_ld();
 #pragma unroll
             for (int j = 0; j < 8; j++)
-                atomicAdd(acc + pos + 8 * hh + j, make_float4(a[4 * j], a[4 * j + 1], a[4 * j + 2], a[4 * j + 3]));
+                red_add_f4(acc + pos + 8 * hh + j, a[4 * j], a[4 * j + 1], a[4 * j + 2], a[4 * j + 3]);
         }
     }
 };
@@ -388,8 +436,10 @@ struct SinkZ {
 struct JobMap {
     long long njobs;   // spectra in this launch
     int len;           // spectra per slot (runs mode) or per blockIdx.y chunk
-    int nslots;        // valid slots (columns / rows / runs)
+    int nslots;        // valid slots (columns / rows / runs x variants)
     int runs_mode;     // 1: slot_id indexes a run of spectra (single); 0: blockIdx.y does
+    int nrun;          // runs mode: number of runs; slot_id = variant * nrun + run (variant 0 only unless the front end
+                       // splits a spectrum over several slots, FrontRawR2)
     long long c0;      // spectrum count since stream start at job 0 (accumulation windows)
     long long M;       // spectra per accumulation window
 };
@@ -418,9 +468,10 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
     const int t = IL ? (tid / G) : (tid % NTS);
     const int slot_id = blockIdx.x * G + slot;
     const bool slot_ok = slot_id < jm.nslots;
-    const long long j0 = (long long)(jm.runs_mode ? slot_id : blockIdx.y) * jm.len;
+    const long long j0 = (long long)(jm.runs_mode ? slot_id % jm.nrun : blockIdx.y) * jm.len;
     const long long j1 = (j0 + jm.len < jm.njobs) ? j0 + jm.len : jm.njobs;
-    const int off = front.off(slot_id);
+    const int off = front.off(jm.runs_mode ? slot_id / jm.nrun : slot_id);
+    const int acc_slot = jm.runs_mode ? slot_id / jm.nrun : slot_id;   // which stretch of the accumulator this slot adds to
 
     // last-stage swizzle of the slot-major layout: RLAST contiguous points per item, so XOR the low
     // bits with the item index to spread a quarter-warp over all banks
@@ -493,24 +544,24 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
     long long wcur = (jm.c0 + j0) / jm.M;
     long long nextb = (wcur + 1) * jm.M - jm.c0;
     static_assert(PL::RLAST == 16, "the last stage is always radix 16 (one put16 per thread and job)");
-    auto flush_all = [&](long long w) { sink.flush(st, slot_id, t, w); };
+    auto flush_all = [&](long long w) { sink.flush(st, acc_slot, t, w); };
 
     // thread 0 issues the copies of iteration `it` for every slot of the CTA
     auto issue = [&](int it) {
         uint32_t bytes = 0;
         for (int g = 0; g < G; g++) {
             const int sid = blockIdx.x * G + g;
-            const long long gj0 = (long long)(jm.runs_mode ? sid : blockIdx.y) * jm.len;
+            const long long gj0 = (long long)(jm.runs_mode ? sid % jm.nrun : blockIdx.y) * jm.len;
             const long long gj1 = (gj0 + jm.len < jm.njobs) ? gj0 + jm.len : jm.njobs;
             if (sid < jm.nslots && gj0 + it < gj1) bytes += XB;
         }
         mbar_expect_tx(bar, bytes);
         for (int g = 0; g < G; g++) {
             const int sid = blockIdx.x * G + g;
-            const long long gj0 = (long long)(jm.runs_mode ? sid : blockIdx.y) * jm.len;
+            const long long gj0 = (long long)(jm.runs_mode ? sid % jm.nrun : blockIdx.y) * jm.len;
             const long long gj1 = (gj0 + jm.len < jm.njobs) ? gj0 + jm.len : jm.njobs;
             if (sid < jm.nslots && gj0 + it < gj1)
-                bulk_g2s(xbuf + (size_t)g * XB, front.src(gj0 + it, front.off(sid)), XB, bar);
+                bulk_g2s(xbuf + (size_t)g * XB, front.src(gj0 + it, front.off(jm.runs_mode ? sid / jm.nrun : sid)), XB, bar);
         }
     };
     if (BULK) {
@@ -539,7 +590,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
                 cpx v[RA];
 #pragma unroll
                 for (int r = 0; r < RA; r++)
-                    v[r] = BULK ? front.decode(xbuf + (size_t)slot * XB, ja + r * LA) : front.load(m, ja + r * LA, off);
+                    v[r] = BULK ? front.decode(xbuf + (size_t)slot * XB, ja + r * LA, off) : front.load(m, ja + r * LA, off);
                 if (DUMP) {
 #pragma unroll
                     for (int r = 0; r < RA; r++) front.dump_put(dump, m, ja + r * LA, off, v[r]);

@@ -59,6 +59,7 @@ struct spec_ctx {
     float2* d_twT = nullptr;     // fused path with N1 > 16: twT[p1*N2 + n2] = W_N^{n2 k1(p1)}
     void* d_tcB = nullptr;       // tensor-core first stage (spec_set_option): split fp16 DFT matrix
     bool tc_stage = false;
+    bool r2_single = false;      // direct FFT, N = 8192: one k_engine launch, 2 x 4096 via FrontRawR2
     float2* d_tw1 = nullptr;     // W_N1^e (pass A engine), N1 entries
     float2* d_tw2 = nullptr;     // W_N2^e (single / pass B engine), N2 entries
     int* d_perm = nullptr;       // position -> natural channel
@@ -361,7 +362,7 @@ static int launch_single_w(spec_ctx* s, const InputView& view, long long m0, lon
     const long long target = (long long)s->numSM * resident * 2 * G;
     const int len = cdiv(nspec, target);
     const int nruns = cdiv(nspec, len);
-    JobMap jm{nspec, len, nruns, 1, c0, s->M};
+    JobMap jm{nspec, len, nruns, 1, nruns, c0, s->M};
     if (s->dump) {   // test hook: the same kernel, front end only
         auto kd = k_engine<PL, false, G, MINB, FrontRaw<MODE_PFB, P, WIN>, Sink, true>;
         int rc = prep_smem(kd, smem);
@@ -398,7 +399,7 @@ static int launch_passA_w(spec_ctx* s, const InputView& view, long long m0, int 
     if (ny > nb) ny = nb;
     const int len = cdiv(nb, ny);
     ny = cdiv(nb, len);
-    JobMap jm{nb, len, s->N2, 0, 0, 1};
+    JobMap jm{nb, len, s->N2, 0, 1, 0, 1};
     if (s->dump) {   // test hook: the same kernel, front end only
         auto kd = k_engine<PL, true, G, 1, FrontRaw<MODE_PFB, P, WIN>, SinkZ, true>;
         int rc = prep_smem(kd, smem);
@@ -438,13 +439,45 @@ static int launch_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
     if (ny > nb) ny = nb;
     const int len = cdiv(nb, ny);
     ny = cdiv(nb, len);
-    JobMap jm{nb, len, s->N1, 0, c0, s->M};
+    JobMap jm{nb, len, s->N1, 0, 1, c0, s->M};
     auto kern = k_engine<PL, false, G, MINB, FrontZ, Sink>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
     {
         ProfScope ps(s, 2, st);
         kern<<<dim3(gx, ny), NT, smem, st>>>(front, sink, jm, s->d_tw2, nullptr);
+    }
+    CK(cudaGetLastError());
+    return 0;
+}
+
+// direct FFT with N = 2 L in ONE k_engine launch: every spectrum is two slots (even / odd channels), FrontRawR2
+template <class PL, int WIN>
+static int launch_single_r2(spec_ctx* s, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
+    typedef SinkStokesTmem Sink;
+    constexpr int G = 1, NT = PL::NTS, MINB = 512 / NT;
+    const size_t smem = (size_t)PL::L * (sizeof(float4) + 8) + 16;
+    FrontRawR2<WIN> front{view, s->d_twN, s->d_coef, s->N, PL::L, 0};
+    Sink sink{s->d_ring, acc_floats(s), s->nring, PL::L, 1};
+    const int resident = blocks_by_smem(smem, MINB);
+    const long long target = (long long)s->numSM * resident * 2 / 2;   // runs (each run is two slots)
+    const int len = cdiv(nspec, target < 1 ? 1 : target);
+    const int nruns = cdiv(nspec, len);
+    JobMap jm{nspec, len, 2 * nruns, 1, nruns, c0, s->M};
+    if (s->dump) {
+        auto kd = k_engine<PL, false, G, MINB, FrontRawR2<WIN>, Sink, true>;
+        int rc = prep_smem(kd, smem);
+        if (rc) return rc;
+        kd<<<dim3(2 * nruns), NT, smem, st>>>(front, sink, jm, s->d_tw2, s->dump);
+        CK(cudaGetLastError());
+        return 0;
+    }
+    auto kern = k_engine<PL, false, G, MINB, FrontRawR2<WIN>, Sink>;
+    int rc = prep_smem(kern, smem);
+    if (rc) return rc;
+    {
+        ProfScope ps(s, 0, st);
+        kern<<<dim3(2 * nruns), NT, smem, st>>>(front, sink, jm, s->d_tw2, nullptr);
     }
     CK(cudaGetLastError());
     return 0;
@@ -537,7 +570,7 @@ static int launch_passA_fir(spec_ctx* s, const InputView& view, long long m0, in
     if (ny > nb) ny = nb;
     const int len = cdiv(nb, ny);
     ny = cdiv(nb, len);
-    JobMap jm{nb, len, s->N2, 0, 0, 1};
+    JobMap jm{nb, len, s->N2, 0, 1, 0, 1};
     auto kern = k_engine<PL, true, G, 1, FrontY, SinkZ>;
     int rc = prep_smem(kern, smem);
     if (rc) return rc;
@@ -796,6 +829,7 @@ static int fused_dispatch(spec_ctx* s, bool query, const InputView& view, long l
 // is done inside the kernels, so a launch may span accumulation windows)
 static int run_spectra(spec_ctx* s, const InputView& v, long long m0, long long nspec, long long c0, cudaStream_t st) {
     if (s->N1 == 1) return run_single(s, v, m0, nspec, c0, st);
+    if (s->r2_single) return s->use_coef ? launch_single_r2<PL4096, 1>(s, v, nspec, c0, st) : launch_single_r2<PL4096, 0>(s, v, nspec, c0, st);
     if (s->fused && (s->mode == SPEC_MODE_PFB || !s->use_coef)) return fused_dispatch(s, false, v, nspec, c0, st);
     for (long long b0 = 0; b0 < nspec; b0 += s->zbatch) {
         const int nb = (int)((nspec - b0 < s->zbatch) ? nspec - b0 : s->zbatch);
@@ -850,7 +884,9 @@ static int create_impl(spec_ctx* s) {
 #ifdef SPEC_TUNING
     if (tuning_int("SPEC_NO_FUSED", 0, 0, 1)) s->fused = false;
 #endif
-    if (s->fused && N <= 65536) { s->N1 = 16; s->N2 = N / 16; }
+    s->r2_single = cc_major == 10 && s->P == 2 && s->mode == SPEC_MODE_FFT && N == 8192;
+    if (s->r2_single) { s->fused = false; s->N1 = 2; s->N2 = N / 2; }
+    else if (s->fused && N <= 65536) { s->N1 = 16; s->N2 = N / 16; }
     else if (s->fused) { s->N2 = 4096; s->N1 = N / 4096; }
     else if (N <= 4096) { s->N1 = 1; s->N2 = N; }
     else if (N <= 65536) { s->N1 = 16; s->N2 = N / 16; }
@@ -927,7 +963,7 @@ static int create_impl(spec_ctx* s) {
             if (rc) return rc;
         }
         // (fused path: two rings, alternating launches may overlap)
-        CK(cudaMalloc(&s->d_Z, (size_t)((s->fused && s->fpdl) ? 2 : 1) * s->zbatch * N * sizeof(float4)));
+        if (!s->r2_single) CK(cudaMalloc(&s->d_Z, (size_t)((s->fused && s->fpdl) ? 2 : 1) * s->zbatch * N * sizeof(float4)));
         if (s->fused && s->N1 > 16) {
             std::vector<float2> wt((size_t)N);
             for (int p1 = 0; p1 < s->N1; p1++) {
@@ -1465,7 +1501,7 @@ extern "C" int spec_debug_fir(spec_t* s, const void* d_blocks, int nspec, float*
     InputView view{nullptr, (const uint8_t*)d_blocks, 0};
     int rc = 0;
     s->dump = d_out;
-    if (s->N1 == 1 || (s->fused && (s->mode == SPEC_MODE_PFB || !s->use_coef))) {
+    if (s->N1 == 1 || s->r2_single || (s->fused && (s->mode == SPEC_MODE_PFB || !s->use_coef))) {
         rc = run_spectra(s, view, 0, nspec, 0, st);
     } else {
         for (long long b0 = 0; b0 < nspec && !rc; b0 += s->zbatch) {
@@ -1505,7 +1541,11 @@ extern "C" int spec_plan_info(const spec_t* s, int* n1, int* n2, char* desc, siz
         const bool pfb = s->mode == SPEC_MODE_PFB;
         int r[3];
         radices(s->N2, r);
-        if (s->N1 == 1)
+        if (s->r2_single)
+            snprintf(desc, desc_len, "k_engine<Plan<%d,%d,%d,%d>,FrontRawR2> one launch, two CTAs per spectrum (even / odd channels from "
+                     "the whole raw block, first radix-2 layer in the front end): unpack%s+FFT+Stokes+accumulate",
+                     s->N2, r[0], r[1], r[2], s->use_coef ? "+window" : "");
+        else if (s->N1 == 1)
             snprintf(desc, desc_len, "k_engine<Plan<%d,%d,%d,%d>> single CTA per spectrum: unpack%s+FFT+Stokes+accumulate",
                      s->N2, r[0], r[1], r[2], pfb ? "+FIR" : (s->use_coef ? "+window" : ""));
         else if (s->fused && (pfb || !s->use_coef))

@@ -85,7 +85,7 @@ def test_indexing_bit_exact_with_single_tap_coefficients(nchan, ntaps, npol, ker
         assert np.array_equal(got[m], want), f"spectrum {m} via {desc}"
 
 
-FRONT_FFT = [(256, 2, "k_engine"), (4096, 2, "k_engine"), (4096, 1, "k_engine"), (8192, 2, "k_fused"),
+FRONT_FFT = [(256, 2, "k_engine"), (4096, 2, "k_engine"), (4096, 1, "k_engine"), (8192, 2, "FrontRawR2"), (16384, 2, "k_fused"),
              (32768, 2, "k_fused"), (65536, 2, "k_fused"), (16384, 1, "k_engine pass A"), (131072, 2, "k_fused"), (262144, 2, "k_fused"), (524288, 2, "k_fused")]
 
 
@@ -101,6 +101,18 @@ def test_unpack_and_indexing_bit_exact_direct_fft_front_end(nchan, npol, kernel)
     if kernel is not None:
         assert kernel in desc, desc
     want = raw.reshape(nspec, nchan, 2 * npol).astype(np.float32)
+    if "FrontRawR2" in desc:
+        # N = 2 L in one launch: the front end hands the L-point transform the first radix-2 layer, [r][e]:
+        # r = 0 the sums x[e] + x[e+L] (small integers: exact), r = 1 the differences times W_N^e
+        L = nchan // 2
+        lo, hi = want[:, :L].astype(np.float64), want[:, L:].astype(np.float64)
+        assert np.array_equal(got[:, :L], (lo + hi).astype(np.float32)), desc
+        w = np.exp(-2j * np.pi * np.arange(L) / nchan)
+        for p in range(npol):
+            dz = ((lo[..., 2 * p] - hi[..., 2 * p]) + 1j * (lo[..., 2 * p + 1] - hi[..., 2 * p + 1])) * w
+            gz = got[:, L:, 2 * p].astype(np.float64) + 1j * got[:, L:, 2 * p + 1]
+            assert np.max(np.abs(gz - dz)) <= 3e-7 * 256 * np.sqrt(2), desc
+        return
     assert np.array_equal(got, want), desc
     assert np.array_equal(got.view(np.uint32), want.view(np.uint32))
 
@@ -260,6 +272,20 @@ def test_split_invariance_many_small_calls():
     for x, y, z in zip(a, b, r):
         compare(x, z)
         compare(y, z)
+
+
+@pytest.mark.parametrize("window", [0, 1])
+def test_parity_direct_fft_8192_single_launch(window):
+    """N = 8192 direct FFT: one k_engine launch, every spectrum as two 4096-point transforms of the first radix-2
+    layer (FrontRawR2); rectangular and Hann windows, windows that straddle ragged runs and three calls."""
+    N, M, nspec = 8192, 29, 133
+    raw = synth.dual_pol_stream(81, nspec * N, [synth.F_CFG1])
+    g, gd = gpu_run(raw, N, 1, 2, FFT, M, window=window, splits=[N * 100, N * 1, N * 32])
+    r, rd = oracle_run(raw, N, 1, 2, FFT, M, window=window)
+    assert gd == rd == nspec and len(g) == len(r) == 4
+    for a, b in zip(g, r):
+        compare(a, b, f"N=8192 single launch window={window}")
+        check_stokes_invariants(a)
 
 
 def test_hann_window_fft_mode_and_default_coefficients():
@@ -459,7 +485,7 @@ def test_sweep_longest_accumulation_2e21_spectra(sweep_refs):
 
 # ---------------------------------------------------------------- NEXT-2: first DFT factor on the tensor cores
 
-@pytest.mark.parametrize("nchan", [8192, 16384, 32768])
+@pytest.mark.parametrize("nchan", [16384, 32768])
 @pytest.mark.parametrize("stream", ["random_bytes", "config1"])
 def test_tensor_core_first_stage_parity(nchan, stream):
     """spec_set_option(SPEC_OPT_TENSOR_CORE_STAGE): the 16-point column DFT of the direct-FFT plans as a tcgen05.mma
@@ -497,7 +523,8 @@ def test_tensor_core_first_stage_parity(nchan, stream):
 
 def test_tensor_core_option_rejected_where_the_plan_has_no_such_stage():
     sp = _sp()
-    for args in ((32768, 8, 2, PFB, 4, 1), (4096, 1, 2, FFT, 4, 0), (65536, 1, 2, FFT, 4, 0), (8192, 1, 1, FFT, 4, 0)):
+    for args in ((32768, 8, 2, PFB, 4, 1), (4096, 1, 2, FFT, 4, 0), (8192, 1, 2, FFT, 4, 0), (65536, 1, 2, FFT, 4, 0),
+                 (16384, 1, 1, FFT, 4, 0)):
         s = sp.Spec(*args)
         with pytest.raises(sp.SpecError) as e:
             s.set_option(sp.OPT_TENSOR_CORE_STAGE, 1)
