@@ -516,6 +516,7 @@ def main():
     p.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     p.add_argument("--tensor-core-stage", action="store_true",
                    help="direct-FFT mode, N = 16384 or 32768: first DFT factor via tcgen05.mma (spec_set_option)")
+    p.add_argument("--probes", action="store_true", help="instruction-throughput probes quoted in DESIGN.md section 6")
     p.add_argument("--sweep", action="store_true", help="configs[4]: all 20 points, resident and streamed")
     p.add_argument("--sweep-log2", type=int, default=31, help="log2 of the time samples per sweep point")
     p.add_argument("--sweep-reps", type=int, default=3)
@@ -524,6 +525,11 @@ def main():
         a.warmup = 3
     if a.impl == "reference":
         run_reference(a)
+    elif a.probes:
+        from paper_1411_0436_b200 import spec as sp
+        for _ in range(3):
+            sp.measure_fp32_peak(0)      # clocks up
+        print(json.dumps({"probes_thread_instructions_per_clk_sm": {n: round(sp.debug_probe(i), 1) for i, n in enumerate(sp.PROBES)}}))
     elif a.sweep:
         run_sweep(a)
     else:

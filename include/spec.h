@@ -181,6 +181,11 @@ int spec_profile_read(spec_t* s, double ms[4], long launches[4]);
 int spec_debug_unpack(const void* d_bytes, size_t nbytes, int npol, float* d_out, void* cuda_stream);
 int spec_debug_fir(spec_t* s, const void* d_blocks, int nspec, float* d_out, void* cuda_stream);
 
+/* Throughput probe behind the design notes: thread-instructions per clock and SM (at the
+ * device's nominal clock) of op 0 scalar FFMA, 1 packed FFMA2, 2 packed FADD2, 3 PRMT, 4 LDS.128 alone,
+ * 5 LDS.128 with eight FFMA2 behind each load (counts the loads), 6 SHFL; 1024 threads per SM, independent chains. */
+int spec_debug_probe(int op, double* out_per_clk_sm, void* cuda_stream);
+
 /* Test hook for the soak test: a foreign kernel of one CTA per SM that holds smem_bytes of shared memory
  * (up to 227 KiB) and spins for about ms milliseconds (at most 2000) on cuda_stream. */
 int spec_debug_hog(int ms, size_t smem_bytes, void* cuda_stream);

@@ -139,6 +139,14 @@ __device__ __forceinline__ void wait_counter_wrap(const unsigned* ctr, unsigned 
     }
 }
 
+// Barrier of a role group: BAR = 0 the whole CTA, BAR > 0 named barrier BAR of 128 threads (k_fused2: a producer
+// group and a consumer group share one CTA)
+template <int BAR>
+__device__ __forceinline__ void gsync() {
+    if (BAR == 0) __syncthreads();
+    else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(128) : "memory");
+}
+
 // ---------------------------------------------------------------- A task, PFB mode
 // C = 16 adjacent columns n2 (all 16 rows n1: 256 filter branches), the GS spectra of one group,
 // R = NT/16 spectra per phase.  The raw samples of a phase (R+7 blocks x 16 rows x 64 bytes) are
@@ -178,7 +186,7 @@ struct ProducerPfb {
 
 // The producer loop of one CTA in PFB mode: tasks rank, rank + NA, ...; `wait_room(g)` (thread 0) returns
 // once the ring slot of group g may be overwritten, `signal(g, next task)` (thread 0) publishes a finished task.
-template <int NT, int N2, bool DUMP, class WaitRoom, class Signal>
+template <int NT, int N2, bool DUMP, class WaitRoom, class Signal, int BAR = 0>
 __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4* smem, int rank, int NA, int natasks,
                                                    WaitRoom wait_room, Signal signal, int lead = 0) {
     typedef ProducerPfb<NT, N2> PP;
@@ -211,7 +219,7 @@ __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4*
         }
         for (int j0 = 0; j0 < nsp; j0 += R) {
             asm volatile("cp.async.wait_all;" ::: "memory");
-            __syncthreads();   // the staged tile is complete; the previous phase's column FFTs have read ysm
+            gsync<BAR>();   // the staged tile is complete; the previous phase's column FFTs have read ysm
             // ---------------- FIR phase
 #pragma unroll
             for (int i = 0; i < BPT; i++) {
@@ -232,7 +240,7 @@ __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4*
                 }
             }
             if (!DUMP && j0 == 0 && tid == lead) wait_room(g);
-            __syncthreads();   // ysm complete, the raw tile is free again
+            gsync<BAR>();   // ysm complete, the raw tile is free again
             // ---------------- stage the next phase (of this task or of my next task)
             if (j0 + R < nsp) PP::stage(p, rawsm, g, tile, j0 + R);
             else if (a + NA < natasks) PP::stage(p, rawsm, (a + NA) >> p.lgTPG, (a + NA) & TPGm, 0);
@@ -257,14 +265,14 @@ __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4*
                 }
             }
         }
-        __syncthreads();   // every Z store of the task has been issued by its thread
+        gsync<BAR>();   // every Z store of the task has been issued by its thread
         if (!DUMP && tid == lead) signal(g, a + NA);
     }
 }
 
 // One A task in direct-FFT mode: no pre-filter, the 16 samples of a column go straight
 // from global memory through the unpack into the butterfly.
-template <int NT, int N2, bool DUMP, class WaitRoom>
+template <int NT, int N2, bool DUMP, class WaitRoom, int BAR = 0>
 __device__ __forceinline__ void fused_task_A_fft(const FusedParams& p, int g, int tile, WaitRoom wait_room, int lead = 0) {
     constexpr int C = 16, R = NT / C, N = 16 * N2;
     const int tid = threadIdx.x;
@@ -278,7 +286,7 @@ __device__ __forceinline__ void fused_task_A_fft(const FusedParams& p, int g, in
 #pragma unroll
     for (int k = 1; k < 16; k++) tw[k] = __ldg(p.twN + (size_t)n2 * k);
     if (!DUMP && tid == lead) wait_room(g);
-    __syncthreads();
+    gsync<BAR>();
     for (int j0 = 0; j0 < nsp; j0 += R) {
         if (j0 + fr < nsp) {
             const uint32_t* base = (const uint32_t*)p.view.in + (size_t)(mg + j0 + fr) * N + n2;
@@ -304,7 +312,7 @@ __device__ __forceinline__ void fused_task_A_fft(const FusedParams& p, int g, in
             }
         }
     }
-    __syncthreads();
+    gsync<BAR>();
 }
 
 // ---------------------------------------------------------------- A task for N1 = 32, 64, 128 (N >= 131072, N2 = 4096)

@@ -18,6 +18,7 @@
 #include "engine.cuh"
 #include "passa_pfb.cuh"
 #include "fused.cuh"
+#include "fused2.cuh"
 
 using namespace spk;
 
@@ -314,6 +315,71 @@ __global__ void __launch_bounds__(1024, 1) k_fp32_peak(float* out, int iters, fl
 #pragma unroll
     for (int i = 0; i < 16; i++) sum += a[i];
     out[blockIdx.x * blockDim.x + threadIdx.x] = sum;
+}
+
+// Throughput probes (spec_debug_probe): thread-instructions per clock and SM of the instruction kinds the kernels are
+// built from, measured with 8-16 independent chains per thread on every SM.  DESIGN.md section 6 quotes them.
+template <int OP>
+__global__ void __launch_bounds__(1024, 1) k_probe(float* out, int iters, float c0, float c1) {
+    extern __shared__ float4 psm[];
+    u64 a[8];
+#pragma unroll
+    for (int i = 0; i < 8; i++) a[i] = pk(threadIdx.x * 1e-9f + i, (float)i);
+    const u64 b = pk(c0 + threadIdx.x * 1e-12f, c0), c = pk(c1, c1);
+    float acc = 0.f;
+    if (OP >= 4 && OP <= 5) {
+        for (int i = threadIdx.x; i < 4096; i += blockDim.x) psm[i] = make_float4((float)i, 1.f, 2.f, 3.f);
+        __syncthreads();
+    }
+    int idx = threadIdx.x;
+    for (int it = 0; it < iters; it++) {
+        if (OP == 0) {          // scalar FFMA, three register operands (16 per iteration)
+#pragma unroll
+            for (int i = 0; i < 8; i++) {
+                float lo, hi;
+                upk(a[i], lo, hi);
+                asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(lo) : "f"(c0), "f"(c1));
+                asm volatile("fma.rn.f32 %0, %0, %1, %2;" : "+f"(hi) : "f"(c0), "f"(c1));
+                a[i] = pk(lo, hi);
+            }
+        } else if (OP == 1) {   // FFMA2 (8)
+#pragma unroll
+            for (int i = 0; i < 8; i++) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(a[i]) : "l"(b), "l"(c));
+        } else if (OP == 2) {   // FADD2, two distinct register pairs (8)
+#pragma unroll
+            for (int i = 0; i < 8; i++) asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(a[i]) : "l"(a[i]), "l"(a[(i + 3) & 7]));
+        } else if (OP == 3) {   // PRMT (16)
+#pragma unroll
+            for (int i = 0; i < 8; i++) {
+                unsigned lo = (unsigned)a[i], hi = (unsigned)(a[i] >> 32);
+                asm volatile("prmt.b32 %0, %0, %1, 0x7440;" : "+r"(lo) : "r"((unsigned)b));
+                asm volatile("prmt.b32 %0, %0, %1, 0x7440;" : "+r"(hi) : "r"((unsigned)b));
+                a[i] = ((u64)hi << 32) | lo;
+            }
+        } else if (OP == 4 || OP == 5) {   // LDS.128 (4), alone or with 8 FFMA2 behind each
+#pragma unroll
+            for (int j = 0; j < 4; j++) {
+                const float4 v = psm[(idx + j * 1024) & 4095];
+                acc += v.x;
+                if (OP == 5) {
+#pragma unroll
+                    for (int i = 0; i < 8; i++) asm volatile("fma.rn.f32x2 %0, %0, %1, %2;" : "+l"(a[i]) : "l"(b), "l"(c));
+                }
+            }
+            idx += 32;
+        } else {                // SHFL: one dual-pol point (four words) to another lane (16 shuffles = 4 points)
+#pragma unroll
+            for (int i = 0; i < 8; i++) {
+                unsigned lo = (unsigned)a[i], hi = (unsigned)(a[i] >> 32);
+                lo = __shfl_xor_sync(0xffffffffu, lo, 1 + (i & 15));
+                hi = __shfl_xor_sync(0xffffffffu, hi, 1 + (i & 15));
+                a[i] = ((u64)hi << 32) | lo;
+            }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 8; i++) { float lo, hi; upk(a[i], lo, hi); acc += lo + hi; }
+    out[blockIdx.x * blockDim.x + threadIdx.x] = acc;
 }
 
 // ------------------------------------------------------------------ launches
@@ -707,6 +773,10 @@ static int fused_alloc_flags(spec_ctx* s, int ngroups) {
 template <class PL, int NT, int MODE_PFB, int PER_SM, int N1 = 16>
 static int fused_do(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
     constexpr bool kTcOk = (MODE_PFB == 0 && N1 == 16 && NT == 128);   // plans that have a tensor-core first stage
+    // plans that run as k_fused2 (both roles per CTA, consumer rows prefetched by bulk copy): direct-FFT mode only.
+    // Measured (profiles/r02_experiments.md): FFT 16384 / 32768 136 -> 149 / 146 GHz, but PFB 32768 117 -> 108 GHz (the
+    // staged rows add a shared-memory pass to a mode whose shared-memory pipe is already half busy with the FIR hand-off)
+    constexpr bool kF2 = (MODE_PFB == 0 && N1 == 16 && NT == 128 && PL::NST == 3);
     auto kern = k_fused<PL, NT, MODE_PFB, PER_SM, false, N1>;
     auto kern_tc = k_fused<PL, NT, MODE_PFB, PER_SM, false, N1, kTcOk>;
     // exchange buffer / FIR hand-off, plus (PFB) the staged raw tile of a producer phase: R+7 blocks of 1 KiB
@@ -721,6 +791,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         int rc = prep_smem(kern, smem);
         if (rc) return rc;
         if (kTcOk) { rc = prep_smem(kern_tc, smem_tc); if (rc) return rc; }
+        if constexpr (kF2) { rc = prep_smem(k_fused2<PL, MODE_PFB>, Fused2Shape<PL, MODE_PFB>::SMEM); if (rc) return rc; }
         // resident CTAs per SM: 128 registers x 512 threads fill the register file, 4 x 64 (2 x 128) TMEM
         // columns and 4 x 33 KB of shared memory fit.  The occupancy API cannot be asked: it reports 1
         // for any kernel that contains tcgen05.alloc (measured: 4 such CTAs of 128 threads do share an
@@ -784,7 +855,11 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         {
             ProfScope ps(s, 0, st);
             if (tc) CK(cudaLaunchKernelEx(&cfg, kern_tc, p));
-            else CK(cudaLaunchKernelEx(&cfg, kern, p));
+            else if constexpr (kF2) {
+                cfg.gridDim = dim3(2 * s->numSM); cfg.blockDim = dim3(256);
+                cfg.dynamicSmemBytes = Fused2Shape<PL, MODE_PFB>::SMEM;
+                CK(cudaLaunchKernelEx(&cfg, k_fused2<PL, MODE_PFB>, p));
+            } else CK(cudaLaunchKernelEx(&cfg, kern, p));
         }
         CK(cudaGetLastError());
         rc = fused_chain_leave(ch, st);
@@ -792,7 +867,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
     }
     // the launch is queued: only now does the handle move on
     s->fpar ^= 1;
-    if (p.carry_chunks) s->carry_cum += (unsigned)s->fgrid;
+    if (p.carry_chunks) s->carry_cum += cfg.gridDim.x;
     return 0;
 }
 
@@ -1479,6 +1554,52 @@ extern "C" int spec_measure_fp32_peak(double* out_tflops, void* cuda_stream) {
     cudaEventDestroy(e1);
     cudaFree(buf);
     *out_tflops = best;
+    return SPEC_OK;
+}
+
+extern "C" int spec_debug_probe(int op, double* out_per_clk_sm, void* cuda_stream) {
+    if (!out_per_clk_sm || op < 0 || op > 6) return SPEC_ERR_ARG;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int dev = 0, nsm = 0, khz = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev));
+    CK(cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, dev));
+    float* buf = nullptr;
+    CK(cudaMalloc(&buf, (size_t)nsm * 1024 * sizeof(float)));
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    const int iters = 8192;
+    static const double per_iter[7] = {16, 8, 8, 16, 4, 4, 16};
+    auto launch = [&](void) {
+        switch (op) {
+            case 0: k_probe<0><<<nsm, 1024, 0, st>>>(buf, iters, 0.999f, 0.001f); break;
+            case 1: k_probe<1><<<nsm, 1024, 0, st>>>(buf, iters, 0.999f, 0.001f); break;
+            case 2: k_probe<2><<<nsm, 1024, 0, st>>>(buf, iters, 0.999f, 0.001f); break;
+            case 3: k_probe<3><<<nsm, 1024, 0, st>>>(buf, iters, 0.999f, 0.001f); break;
+            case 4: k_probe<4><<<nsm, 1024, 65536, st>>>(buf, iters, 0.999f, 0.001f); break;
+            case 5: k_probe<5><<<nsm, 1024, 65536, st>>>(buf, iters, 0.999f, 0.001f); break;
+            default: k_probe<6><<<nsm, 1024, 0, st>>>(buf, iters, 0.999f, 0.001f); break;
+        }
+    };
+    CK(cudaFuncSetAttribute(k_probe<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536));
+    CK(cudaFuncSetAttribute(k_probe<5>, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536));
+    double best = 0.0;
+    for (int rep = 0; rep < 3; rep++) {
+        CK(cudaEventRecord(e0, st));
+        launch();
+        CK(cudaEventRecord(e1, st));
+        CK(cudaEventSynchronize(e1));
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, e0, e1));
+        const double v = per_iter[op] * iters * 1024.0 / (ms * 1e-3) / ((double)khz * 1e3);
+        if (rep > 0 && v > best) best = v;
+    }
+    CK(cudaGetLastError());
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(buf);
+    *out_per_clk_sm = best;
     return SPEC_OK;
 }
 

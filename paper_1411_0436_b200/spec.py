@@ -27,7 +27,7 @@ SYMBOLS = [
     "spec_stream_host", "spec_measure_fp32_peak", "spec_debug_unpack", "spec_debug_fir",
     "spec_strerror", "spec_last_error", "spec_profile", "spec_profile_read", "spec_read_accum_batch",
     "spec_plan_info", "spec_debug_hog", "spec_set_option", "spec_capture_begin", "spec_capture_end", "spec_replayed",
-    "spec_accumulate_host", "spec_create_subbands",
+    "spec_accumulate_host", "spec_create_subbands", "spec_debug_probe",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -55,6 +55,7 @@ _lib.spec_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), _vp]
 _lib.spec_debug_unpack.argtypes = [_vp, _sz, C.c_int, _vp, _vp]
 _lib.spec_debug_fir.argtypes = [_vp, _vp, C.c_int, _vp, _vp]
 _lib.spec_debug_hog.argtypes = [C.c_int, _sz, _vp]
+_lib.spec_debug_probe.argtypes = [C.c_int, C.POINTER(C.c_double), _vp]
 _lib.spec_set_option.argtypes = [_vp, C.c_int, C.c_int]
 _lib.spec_capture_begin.argtypes = [_vp]
 _lib.spec_capture_end.argtypes = [_vp]
@@ -94,6 +95,16 @@ def measure_fp32_peak(stream=0):
 
 def debug_unpack(d_bytes_ptr, nbytes, d_out_ptr, stream=0, npol=2):
     _check(_lib.spec_debug_unpack(d_bytes_ptr, nbytes, npol, d_out_ptr, stream), "spec_debug_unpack")
+
+
+PROBES = ("FFMA", "FFMA2", "FADD2", "PRMT", "LDS.128", "LDS.128 with 8 FFMA2 each", "SHFL")
+
+
+def debug_probe(op, stream=0):
+    """Thread-instructions per clock and SM of instruction kind PROBES[op]."""
+    out = C.c_double(0.0)
+    _check(_lib.spec_debug_probe(op, C.byref(out), stream), "spec_debug_probe")
+    return out.value
 
 
 def debug_hog(ms, smem_bytes, stream=0):
