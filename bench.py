@@ -14,8 +14,8 @@ the whole chain unpack -> FIR -> FFT -> Stokes -> accumulate -> read-out.
 
 `value`  : inputs resident in HBM before the timed region.
 `e2e`    : the same work through spec_stream_host from PINNED HOST memory (H2D inside the timed
-           region, double-buffered on a side stream) plus a device-to-host read of every completed
-           accumulation.
+           region, double-buffered on a side stream) plus a device-to-host copy of every completed
+           accumulation into pinned host memory (on a third stream, inside the timed region).
 `roofline`: dominant kernel's nominal fp32 flops / its time vs the fp32 peak measured in this run
            (spec_measure_fp32_peak).  Where one kernel is the whole chain its time is taken from the timed
            pass itself ((step time - read-out kernels) / launches: the launches overlap there, no event sits
@@ -142,9 +142,10 @@ def workload_from_args(a):
     nchan = a.nchan
     ntaps = 8 if pfb else 1
     chunk_samples = CHUNK_BYTES // 4
-    nacc = a.nacc if a.nacc else (256 if nchan == 32768 and pfb else max(1, chunk_samples // nchan // 2))
-    name = ("configs[1]: dual-pol PFB N=32768 T=8 M=256, 64 MiB calls" if (pfb and nchan == 32768 and nacc == 256)
-            else f"dual-pol {'PFB T=8' if pfb else 'direct FFT'} N={nchan} M={nacc}, 64 MiB calls")
+    nacc = a.nacc if a.nacc else (256 if nchan == 32768 and pfb else max(1, chunk_samples // a.nsub // nchan // 2))
+    name = ("configs[1]: dual-pol PFB N=32768 T=8 M=256, 64 MiB calls" if (pfb and nchan == 32768 and nacc == 256 and a.nsub == 1)
+            else f"dual-pol {'PFB T=8' if pfb else 'direct FFT'} N={nchan} M={nacc}, 64 MiB calls"
+                 + (f", {a.nsub} interleaved sub-bands (value = dual-pol samples/s summed over the sub-bands)" if a.nsub > 1 else ""))
     return dict(pfb=pfb, nchan=nchan, ntaps=ntaps, nacc=nacc, chunk_samples=chunk_samples, name=name)
 
 
@@ -266,7 +267,10 @@ def run_ours(a):
     d_in = h_pinned.to(device, non_blocking=False)
     stream = torch.cuda.current_stream().cuda_stream
 
-    s = sp.Spec(N, T, 2, sp.MODE_PFB if pfb else sp.MODE_FFT, M, sp.WINDOW_HANN if pfb else sp.WINDOW_RECT)
+    K = a.nsub                     # eight-sub-band modes: the same bytes are K interleaved sub-bands of cs / K time samples
+    cs //= K
+    pass_samples //= K
+    s = sp.Spec(N, T, 2, sp.MODE_PFB if pfb else sp.MODE_FFT, M, sp.WINDOW_HANN if pfb else sp.WINDOW_RECT, nsub=K)
     if a.tensor_core_stage:
         s.set_option(sp.OPT_TENSOR_CORE_STAGE, 1)
     n1, n2, plan_desc = s.plan_info()
@@ -276,7 +280,7 @@ def run_ours(a):
     # stay adjacent in the stream and may overlap; the ring holds what completes meanwhile
     ring = max(8, READOUT_EVERY * CALLS_PER_PASS * (cs // N // M + 1) + 2)
     s.set_ring(ring)
-    d_out = torch.empty((ring, 4, N), dtype=torch.float32, device=device)
+    d_out = torch.empty((ring, K * 4, N), dtype=torch.float32, device=device)
     fp32_peak = sp.measure_fp32_peak(stream)
 
     npass = [0]
@@ -284,23 +288,48 @@ def run_ours(a):
     def pass_resident():
         nout = 0
         for c in range(CALLS_PER_PASS):
-            s.process(d_in.data_ptr() + c * cs * 4, cs, stream)
+            s.process(d_in.data_ptr() + c * cs * 4 * K, cs, stream)
         npass[0] += 1
         if npass[0] % READOUT_EVERY == 0:
             while s.pending():
                 nout += s.read_accum_batch_device(d_out.data_ptr(), ring, stream)
         return nout
 
+    # e2e read-back: completed accumulations are popped into one of two device buffers and copied to pinned host
+    # memory on a third stream, so that the device-to-host copy of pass i overlaps the host-to-device copies and the
+    # kernels of pass i+1 (the host link is full duplex)
+    d2h = torch.cuda.Stream(device=device)
+    ring_e = max(8, CALLS_PER_PASS * (cs // N // M + 1) + 2)
+    d_oute = [torch.empty((ring_e, K * 4, N), dtype=torch.float32, device=device) for _ in range(2)]
+    h_oute = [torch.empty((ring_e, K * 4, N), dtype=torch.float32).pin_memory() for _ in range(2)]
+    ev_popped = [torch.cuda.Event() for _ in range(2)]
+    ev_copied = [torch.cuda.Event() for _ in range(2)]
+    epass = [0]
+
     def pass_e2e():
-        nout = 0
+        k = epass[0] & 1
+        epass[0] += 1
+        main = torch.cuda.current_stream()
         s.stream_host(h_pinned.data_ptr(), pass_samples, cs, stream)
-        while s.pending():
-            s.read_accum_host(stream)
-            nout += 1
+        main.wait_event(ev_copied[k])            # buffer k's previous contents have reached the host
+        nout = 0
+        while s.pending() and nout < ring_e:
+            nout += s.read_accum_batch_device(d_oute[k].data_ptr() + nout * 16 * N * K, ring_e - nout, stream)
+        ev_popped[k].record(main)
+        d2h.wait_event(ev_popped[k])
+        with torch.cuda.stream(d2h):
+            h_oute[k][:nout].copy_(d_oute[k][:nout], non_blocking=True)
+            ev_copied[k].record(d2h)
         return nout
 
+    def drain():
+        while s.pending():
+            s.read_accum_batch_device(d_out.data_ptr(), ring, stream)
+        npass[0] = 0
+
     def one_pass_ms(fn, reps=3):
-        fn()
+        for _ in range(reps):
+            fn()
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         e0.record()
@@ -311,6 +340,7 @@ def run_ours(a):
         return e0.elapsed_time(e1) / reps
 
     def timed(fn, passes, steps, warmup, profile):
+        drain()
         for _ in range(warmup):
             for _ in range(passes):
                 fn()
@@ -323,6 +353,7 @@ def run_ours(a):
         for _ in range(steps):
             for _ in range(passes):
                 nout += fn()
+        torch.cuda.current_stream().wait_stream(d2h)   # (e2e: the last read-back is inside the timed region)
         e1.record()
         barrier()
         t1 = time.time()
@@ -348,10 +379,10 @@ def run_ours(a):
     ms_e2e, nout_e2e, prof_e2e, _ = timed(pass_e2e, p_e2e, a.steps, max(1, a.warmup // 2), False)
     s.close()
 
-    step_samples = pass_samples * p_res
+    step_samples = pass_samples * p_res * K        # dual-pol samples over all sub-bands
     total_samples = step_samples * a.steps * ws
     value = total_samples / (ms * 1e-3) / 1e9
-    e2e_step_samples = pass_samples * p_e2e
+    e2e_step_samples = pass_samples * p_e2e * K
     e2e = e2e_step_samples * a.steps * ws / (ms_e2e * 1e-3) / 1e9
 
     # dominant kernel and its roofline (per-launch averages)
@@ -396,7 +427,7 @@ def run_ours(a):
                    "parallelism": f"replicas x{ws}" if ws > 1 else "single GPU",
                    "paper_context": "GTX TITAN: 1.1 GHz (PFB) / 1.4 GHz (FFT) dual-pol, PAPER.md:7"},
         "e2e": {"value": e2e, "unit": "GHz", "h2d_bytes_per_step": e2e_step_samples * 4,
-                "d2h_bytes_per_step": int(nout_e2e / a.steps * 16 * N), "ms_per_step": ms_e2e / a.steps,
+                "d2h_bytes_per_step": int(nout_e2e / a.steps * 16 * N * K), "ms_per_step": ms_e2e / a.steps,
                 "passes_per_step": p_e2e, "h2d_gbs": e2e_step_samples * 4 * a.steps / (ms_e2e * 1e-3) / 1e9},
         "gpu_launches": int(launches),
         "clocks": clocks,
@@ -405,6 +436,7 @@ def run_ours(a):
                      "traffic_note": "dram bytes read+write per launch from the ncu --set full capture listed in "
                                      "profiles/traffic.json (algorithmic: 4 B per dual-pol sample)",
                      "algorithmic_bytes_per_launch": 4 * cs,
+                     "launches_note": (f"{K} sub-bands: one launch per sub-band and call, {cs} samples each" if K > 1 else None),
                      "peak_source": "spec_measure_fp32_peak in this run (FFMA chains, all SMs); "
                                     "MEASURED_PEAKS.json has no fp32 figure",
                      "peak_nominal": NOMINAL_FP32_TFLOPS, "launches": int(launches0[kern]),
@@ -504,6 +536,65 @@ def run_sweep(a):
           f"resident: median of {a.sweep_reps} runs.")
 
 
+def run_packets(a):
+    """the real-time ingest shape, many small calls.  A periodic segment of 18
+    spec_process calls of 8 blocks each plus its three batched read-outs, issued call by call and as ONE CUDA graph."""
+    from paper_1411_0436_b200 import spec as sp
+    from paper_1411_0436_b200 import synth
+    torch, rank, local_rank, ws, device, dist = _setup_device()
+    if rank != 0:
+        return
+    pfb = a.mode == "pfb"
+    N, T, M, bpc, ncalls = a.nchan, (8 if pfb else 1), 16, 8, 18
+    seg = bpc * ncalls * N
+    raw = synth.dual_pol_stream(synth.SEED_BASE + 5, (T - 1) * N + seg, [synth.F_CFG1])
+    d_all = torch.from_numpy(raw.reshape(-1)).to(device)
+    d_seg = d_all[(T - 1) * N * 4:]
+    d_out = torch.zeros((9, 4, N), dtype=torch.float32, device=device)
+    res = {}
+    for use_graph in (False, True):
+        s = sp.Spec(N, T, 2, sp.MODE_PFB if pfb else sp.MODE_FFT, M, sp.WINDOW_HANN if pfb else sp.WINDOW_RECT)
+        if T > 1:
+            s.process(d_all.data_ptr(), (T - 1) * N, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+
+        def segment(st):
+            got = 0
+            for c in range(ncalls):
+                s.process(d_seg.data_ptr() + c * bpc * N * 4, bpc * N, st)
+                if c % 6 == 5:
+                    got += s.read_accum_batch_device(d_out.data_ptr() + got * 16 * N, 8, st)
+            return got
+
+        if use_graph:
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g):
+                s.capture_begin()
+                segment(torch.cuda.current_stream().cuda_stream)
+                s.capture_end()
+            run = g.replay
+        else:
+            run = lambda: segment(torch.cuda.current_stream().cuda_stream)
+        for _ in range(20):
+            run()
+        torch.cuda.synchronize()
+        reps = 200
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0 = time.perf_counter()
+        e0.record()
+        for _ in range(reps):
+            run()
+        e1.record()
+        torch.cuda.synchronize()
+        wall = time.perf_counter() - t0
+        ms = e0.elapsed_time(e1)
+        res["graph" if use_graph else "calls"] = {"us_per_call_device": ms * 1e3 / (reps * ncalls), "us_per_call_host": wall * 1e6 / (reps * ncalls),
+                                                   "ghz": reps * bpc * ncalls * N / (ms * 1e-3) / 1e9}
+        s.close()
+    print(json.dumps({"packets": True, "mode": a.mode, "nchan": N, "blocks_per_call": bpc, "calls_per_segment": ncalls,
+                      "samples_per_call": bpc * N, **res}))
+
+
 def main():
     p = argparse.ArgumentParser()
     p.add_argument("--gpus", type=int, default=1)
@@ -514,6 +605,9 @@ def main():
     p.add_argument("--mode", default="pfb", choices=["pfb", "fft"])
     p.add_argument("--nacc", type=int, default=0)
     p.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    p.add_argument("--nsub", type=int, default=1, help="eight-sub-band modes (PAPER.md:73): interleaved sub-bands per time sample")
+    p.add_argument("--packets", action="store_true",
+                   help="NEXT-4: packet-sized calls (8 blocks each), issued one by one and replayed as one CUDA graph")
     p.add_argument("--tensor-core-stage", action="store_true",
                    help="direct-FFT mode, N = 16384 or 32768: first DFT factor via tcgen05.mma (spec_set_option)")
     p.add_argument("--probes", action="store_true", help="instruction-throughput probes quoted in DESIGN.md section 6")
@@ -530,6 +624,8 @@ def main():
         for _ in range(3):
             sp.measure_fp32_peak(0)      # clocks up
         print(json.dumps({"probes_thread_instructions_per_clk_sm": {n: round(sp.debug_probe(i), 1) for i, n in enumerate(sp.PROBES)}}))
+    elif a.packets:
+        run_packets(a)
     elif a.sweep:
         run_sweep(a)
     else:

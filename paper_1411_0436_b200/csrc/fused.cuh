@@ -141,10 +141,10 @@ __device__ __forceinline__ void wait_counter_wrap(const unsigned* ctr, unsigned 
 
 // Barrier of a role group: BAR = 0 the whole CTA, BAR > 0 named barrier BAR of 128 threads (k_fused2: a producer
 // group and a consumer group share one CTA)
-template <int BAR>
+template <int BAR, int CNT = 128>
 __device__ __forceinline__ void gsync() {
     if (BAR == 0) __syncthreads();
-    else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(128) : "memory");
+    else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(CNT) : "memory");
 }
 
 // ---------------------------------------------------------------- A task, PFB mode
@@ -219,7 +219,7 @@ __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4*
         }
         for (int j0 = 0; j0 < nsp; j0 += R) {
             asm volatile("cp.async.wait_all;" ::: "memory");
-            gsync<BAR>();   // the staged tile is complete; the previous phase's column FFTs have read ysm
+            gsync<BAR, NT>();   // the staged tile is complete; the previous phase's column FFTs have read ysm
             // ---------------- FIR phase
 #pragma unroll
             for (int i = 0; i < BPT; i++) {
@@ -240,7 +240,7 @@ __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4*
                 }
             }
             if (!DUMP && j0 == 0 && tid == lead) wait_room(g);
-            gsync<BAR>();   // ysm complete, the raw tile is free again
+            gsync<BAR, NT>();   // ysm complete, the raw tile is free again
             // ---------------- stage the next phase (of this task or of my next task)
             if (j0 + R < nsp) PP::stage(p, rawsm, g, tile, j0 + R);
             else if (a + NA < natasks) PP::stage(p, rawsm, (a + NA) >> p.lgTPG, (a + NA) & TPGm, 0);
@@ -265,7 +265,7 @@ __device__ __forceinline__ void fused_producer_pfb(const FusedParams& p, float4*
                 }
             }
         }
-        gsync<BAR>();   // every Z store of the task has been issued by its thread
+        gsync<BAR, NT>();   // every Z store of the task has been issued by its thread
         if (!DUMP && tid == lead) signal(g, a + NA);
     }
 }
@@ -286,7 +286,7 @@ __device__ __forceinline__ void fused_task_A_fft(const FusedParams& p, int g, in
 #pragma unroll
     for (int k = 1; k < 16; k++) tw[k] = __ldg(p.twN + (size_t)n2 * k);
     if (!DUMP && tid == lead) wait_room(g);
-    gsync<BAR>();
+    gsync<BAR, NT>();
     for (int j0 = 0; j0 < nsp; j0 += R) {
         if (j0 + fr < nsp) {
             const uint32_t* base = (const uint32_t*)p.view.in + (size_t)(mg + j0 + fr) * N + n2;
@@ -312,7 +312,7 @@ __device__ __forceinline__ void fused_task_A_fft(const FusedParams& p, int g, in
             }
         }
     }
-    gsync<BAR>();
+    gsync<BAR, NT>();
 }
 
 // ---------------------------------------------------------------- A task for N1 = 32, 64, 128 (N >= 131072, N2 = 4096)
@@ -358,7 +358,7 @@ struct ProducerBig {
     }
 };
 
-template <int NT, int N2, int N1, int T, bool DUMP, class WaitRoom, class Signal>
+template <int NT, int N2, int N1, int T, bool DUMP, class WaitRoom, class Signal, int BAR = 0>
 __device__ __forceinline__ void fused_producer_big(const FusedParams& p, float4* smem, int rank, int NA, int natasks,
                                                    WaitRoom wait_room, Signal signal, int lead) {
     typedef ProducerBig<NT, N2, N1, T> PP;
@@ -384,7 +384,7 @@ __device__ __forceinline__ void fused_producer_big(const FusedParams& p, float4*
             for (int qb = 0; qb < 16; qb++) tw[qb] = __ldg(p.twT + (size_t)(qa * 16 + qb) * N2 + n2_0 + c2);
         }
         asm volatile("cp.async.wait_all;" ::: "memory");
-        __syncthreads();   // the staged tile is complete; the previous task's second stage has read ysm
+        gsync<BAR, NT>();   // the staged tile is complete; the previous task's second stage has read ysm
         // ---------------- FIR phase (T = 1: unpack only)
 #pragma unroll
         for (int i = 0; i < BPT; i++) {
@@ -414,7 +414,7 @@ __device__ __forceinline__ void fused_producer_big(const FusedParams& p, float4*
             }
         }
         if (!DUMP && tid == lead) wait_room(g);
-        __syncthreads();   // ysm complete, the raw tile is free again
+        gsync<BAR, NT>();   // ysm complete, the raw tile is free again
         if (a + NA < natasks) PP::stage(p, rawsm, (a + NA) >> p.lgTPG, (a + NA) & TPGm);
         if (DUMP) {   // test hook: what the column transform is about to consume, in the caller's layout
             if (r2 < nsp) {
@@ -443,7 +443,7 @@ __device__ __forceinline__ void fused_producer_big(const FusedParams& p, float4*
                     y0[q * 16 * C] = cpx_to_f4(cmul(v[q], w.x, w.y));
                 }
             }
-            __syncthreads();
+            gsync<BAR, NT>();
             // ---------------- second stage: radix 16 over block qa, W_N^{n2 k1}, rows p1 = 16 qa + qb of the Z ring
             if (r2 < nsp) {
                 cpx v[16];
@@ -455,7 +455,7 @@ __device__ __forceinline__ void fused_producer_big(const FusedParams& p, float4*
                 for (int qb = 0; qb < 16; qb++) zp[(size_t)qb * N2] = cpx_to_f4(cmul(v[qb], tw[qb].x, tw[qb].y));
             }
         }
-        __syncthreads();   // every Z store of the task has been issued by its thread; ysm may be overwritten
+        gsync<BAR, NT>();   // every Z store of the task has been issued by its thread; ysm may be overwritten
         if (!DUMP && tid == lead) signal(g, a + NA);
     }
 }

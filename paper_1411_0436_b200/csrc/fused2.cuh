@@ -20,25 +20,32 @@
 
 namespace spk {
 
-template <class PL, int MODE_PFB>
+// NT = threads per role group: 128 (N2 <= 2048, two CTAs per SM) or 256 (N2 = 4096: N = 65536 and, with the
+// N1 = 32 / 64 / 128 column plans of ProducerBig, N >= 131072; one CTA of 512 threads per SM)
+template <class PL, int MODE_PFB, int N1>
 struct Fused2Shape {
-    static constexpr int NT = 128;                                   // threads per role group
+    static constexpr int NT = (PL::L == 4096) ? 256 : 128;
     static constexpr int G = NT / PL::NTS;                           // rows per B job
-    static constexpr size_t P_BYTES = MODE_PFB ? (size_t)NT * 16 * sizeof(float4) + (size_t)(NT / 16 + 7) * 1024 : 0;
-    static constexpr size_t ROW_BYTES = (size_t)G * PL::L * sizeof(float4);   // one job's rows: 32 KB
+    static constexpr size_t P16 = MODE_PFB ? (size_t)NT * 16 * sizeof(float4) + (size_t)(NT / 16 + 7) * 1024 : 0;
+    static constexpr size_t PBIG = ProducerBig<256, PL::L, (N1 > 16 ? N1 : 32), MODE_PFB ? 8 : 1>::SMEM;
+    static constexpr size_t P_BYTES = (N1 > 16) ? PBIG : P16;
+    static constexpr size_t ROW_BYTES = (size_t)G * PL::L * sizeof(float4);   // one job's rows: 32 or 64 KB
     static constexpr size_t SMEM = P_BYTES + 2 * ROW_BYTES;
+    static constexpr bool kFits = SMEM + 2048 <= 227 * 1024 / (256 / NT);
 };
 
-template <class PL, int MODE_PFB>
-__global__ void __launch_bounds__(256, 2)
+template <class PL, int MODE_PFB, int N1 = 16>
+__global__ void __launch_bounds__(2 * Fused2Shape<PL, MODE_PFB, N1>::NT, 256 / Fused2Shape<PL, MODE_PFB, N1>::NT)
 k_fused2(const FusedParams p) {
-    typedef Fused2Shape<PL, MODE_PFB> SH;
+    typedef Fused2Shape<PL, MODE_PFB, N1> SH;
     constexpr int NT = SH::NT;
+    constexpr int NTC = 2 * NT;                     // threads per CTA
+    constexpr int TCOLS = 2 * NT;                   // tensor-memory columns: the consumer warps use the upper half
     constexpr int L = PL::L, RA = PL::RA, RB = PL::RB, RC = PL::RC, NST = PL::NST;
     constexpr int LA = PL::LA, LB = PL::LB, NTS = PL::NTS;
     constexpr int G = SH::G;
-    constexpr int RGN = 16 / G;                     // row groups per spectrum
-    static_assert(NST == 3 && LB == 16 && RB == 16 && RC == 16 && LA % 128 == 0 && G >= 1 && G < 16, "three-stage row plan");
+    constexpr int RGN = N1 / G;                     // row groups per spectrum (a spectrum has N1 rows)
+    static_assert(NST == 3 && LB == 16 && RB == 16 && RC == 16 && LA % 128 == 0 && G >= 1 && G < N1, "three-stage row plan");
     extern __shared__ float4 smem[];
     float4* const rowbuf = (float4*)((uint8_t*)smem + SH::P_BYTES);   // [2][G*L]
     __shared__ uint32_t s_tmem;
@@ -52,10 +59,10 @@ k_fused2(const FusedParams p) {
     const int ngroups = (p.nspec + GS - 1) >> p.lgGS;
     const unsigned TPG = 1u << p.lgTPG;
     const unsigned a_full = TPG;
-    const unsigned rows_full = (unsigned)GS * 16u;
+    const unsigned rows_full = (unsigned)GS * (unsigned)N1;
 
-    // 256 columns: SinkStokesTmem addresses column block (warp >> 2), i.e. the consumer warps 4-7 use columns 128..255
-    const uint32_t tmem_base = tmem_alloc_cta<256>(&s_tmem);
+    // SinkStokesTmem addresses column block (warp >> 2) of 128 columns: the consumer warps use the upper half
+    const uint32_t tmem_base = tmem_alloc_cta<TCOLS>(&s_tmem);
     if (gtid == 0) {
         mbar_init(&s_full[0], 1);
         mbar_init(&s_full[1], 1);
@@ -64,7 +71,7 @@ k_fused2(const FusedParams p) {
             fence_acquire_gpu();
         }
     }
-    for (int i = blockIdx.x * 256 + gtid; i < p.carry_chunks; i += gridDim.x * 256) p.carry_dst[i] = __ldg(p.carry_src + i);
+    for (int i = blockIdx.x * NTC + gtid; i < p.carry_chunks; i += gridDim.x * NTC) p.carry_dst[i] = __ldg(p.carry_src + i);
     __syncthreads();
     if (p.carry_chunks && gtid == 0) red_release_u32(p.carry_cnt, 1u);
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -95,7 +102,11 @@ k_fused2(const FusedParams p) {
             red_release_u32(p.a_done + g, 1u);   // all Z stores of the group are ordered before it
             prefetch_room(a_next);
         };
-        if (MODE_PFB) {
+        if constexpr (N1 > 16) {
+            if (tid == 0) prefetch_room(rank);
+            fused_producer_big<NT, L, N1, MODE_PFB ? 8 : 1, false, decltype(wait_room), decltype(signal), 1>(
+                p, smem, rank, ngrp, natasks, wait_room, signal, 0);
+        } else if (MODE_PFB) {
             if (tid == 0) prefetch_room(rank);
             fused_producer_pfb<NT, L, false, decltype(wait_room), decltype(signal), 1>(p, smem, rank, ngrp, natasks, wait_room, signal, 0);
         } else {
@@ -173,7 +184,7 @@ k_fused2(const FusedParams p) {
         auto issue_rows = [&](int b, int zp) {
             asm volatile("fence.proxy.async.global;" ::: "memory");   // the producers' stores -> this copy's reads
             mbar_expect_tx(&s_full[b], (uint32_t)SH::ROW_BYTES);
-            bulk_g2s(rowbuf + (size_t)b * G * L, p.Z + (size_t)zp * (16 * L) + (size_t)(rg * G) * L, (uint32_t)SH::ROW_BYTES, &s_full[b]);
+            bulk_g2s(rowbuf + (size_t)b * G * L, p.Z + (size_t)zp * (N1 * L) + (size_t)(rg * G) * L, (uint32_t)SH::ROW_BYTES, &s_full[b]);
         };
         if (tid == 0 && nbj > 0) {
             prefetch_ready(0);
@@ -181,7 +192,7 @@ k_fused2(const FusedParams p) {
             issue_rows(0, zpos);
             prefetch_ready(1);
         }
-        gsync<2>();
+        gsync<2, NT>();
         for (int bi = 0; bi < nbj; bi++) {
             const int b = bi & 1;
             float4* const buf = rowbuf + (size_t)b * G * L;
@@ -214,7 +225,7 @@ k_fused2(const FusedParams p) {
             // the rows are in shared memory: their ring lines are dead (drop them from the L2 instead of letting them
             // be written back) and the producers may reuse the slot
             {
-                const float4* zrow = p.Z + (size_t)zpos * (16 * L) + (size_t)row * L;
+                const float4* zrow = p.Z + (size_t)zpos * (N1 * L) + (size_t)row * L;
 #pragma unroll
                 for (int i = 0; i < (L * 16) / (NTS * 128); i++)
                     asm volatile("discard.global.L2 [%0], 128;" ::"l"(zrow + (t + NTS * i) * 8) : "memory");
@@ -225,7 +236,7 @@ k_fused2(const FusedParams p) {
                 red_release_u32(p.b_done + (m >> p.lgGS), (unsigned)G);
                 if (bi + 1 < nbj) { wait_ready(bi + 1); prefetch_ready(bi + 2); }
             }
-            gsync<2>();
+            gsync<2, NT>();
             // every thread is past stage c of the previous job: its buffer takes the next job's rows
             if (tid == 0 && bi + 1 < nbj) issue_rows(b ^ 1, zn);
             // ---------------- stage b (in place per thread), stage c, Stokes into tensor memory
@@ -269,10 +280,10 @@ k_fused2(const FusedParams p) {
     __syncthreads();
     if (s_last) {
         __threadfence();
-        for (int i = gtid; i < ngroups; i += 256) { p.a_done[i] = 0u; p.b_done[i] = 0u; }
-        for (int i = gtid; i < kFusedRoleWords; i += 256) p.role[i] = 0u;
+        for (int i = gtid; i < ngroups; i += NTC) { p.a_done[i] = 0u; p.b_done[i] = 0u; }
+        for (int i = gtid; i < kFusedRoleWords; i += NTC) p.role[i] = 0u;
     }
-    if (gtid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(256) : "memory");
+    if (gtid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TCOLS) : "memory");
 }
 
 }  // namespace spk

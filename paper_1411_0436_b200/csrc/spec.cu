@@ -684,6 +684,9 @@ static int run_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
 #define B_CASE(LEN, PLX)                                                   \
     case LEN:                                                              \
         return (s->P == 2) ? launch_passB<PLX, 2>(s, nb, c0, st) : launch_passB<PLX, 1>(s, nb, c0, st);
+        B_CASE(64, PL64)
+        B_CASE(128, PL128)
+        B_CASE(256, PL256)
         B_CASE(512, PL512)
         B_CASE(1024, PL1024)
         B_CASE(2048, PL2048)
@@ -773,10 +776,12 @@ static int fused_alloc_flags(spec_ctx* s, int ngroups) {
 template <class PL, int NT, int MODE_PFB, int PER_SM, int N1 = 16>
 static int fused_do(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
     constexpr bool kTcOk = (MODE_PFB == 0 && N1 == 16 && NT == 128);   // plans that have a tensor-core first stage
-    // plans that run as k_fused2 (both roles per CTA, consumer rows prefetched by bulk copy): direct-FFT mode only.
-    // Measured (profiles/r02_experiments.md): FFT 16384 / 32768 136 -> 149 / 146 GHz, but PFB 32768 117 -> 108 GHz (the
-    // staged rows add a shared-memory pass to a mode whose shared-memory pipe is already half busy with the FIR hand-off)
-    constexpr bool kF2 = (MODE_PFB == 0 && N1 == 16 && NT == 128 && PL::NST == 3);
+    // plans that run as k_fused2 (both roles per CTA, consumer rows prefetched by bulk copy): direct-FFT mode, and PFB mode
+    // where rows are 4096 points (N >= 65536: the ring misses the L2 there and the prefetch hides DRAM latency) and the
+    // producer's buffers leave room for two row buffers.  Measured (profiles/r02_experiments.md): FFT 16384 / 32768
+    // 136 -> 149 / 146 GHz, PFB 131072 / 262144 71 -> 82 / 58 -> 71 GHz, but PFB 32768 117 -> 108 GHz (the staged rows add a
+    // shared-memory pass to a mode whose shared-memory pipe is already half busy with the FIR hand-off)
+    constexpr bool kF2 = PL::NST == 3 && Fused2Shape<PL, MODE_PFB, N1>::kFits && (MODE_PFB == 0 || NT == 256);
     auto kern = k_fused<PL, NT, MODE_PFB, PER_SM, false, N1>;
     auto kern_tc = k_fused<PL, NT, MODE_PFB, PER_SM, false, N1, kTcOk>;
     // exchange buffer / FIR hand-off, plus (PFB) the staged raw tile of a producer phase: R+7 blocks of 1 KiB
@@ -791,7 +796,7 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
         int rc = prep_smem(kern, smem);
         if (rc) return rc;
         if (kTcOk) { rc = prep_smem(kern_tc, smem_tc); if (rc) return rc; }
-        if constexpr (kF2) { rc = prep_smem(k_fused2<PL, MODE_PFB>, Fused2Shape<PL, MODE_PFB>::SMEM); if (rc) return rc; }
+        if constexpr (kF2) { rc = prep_smem(k_fused2<PL, MODE_PFB, N1>, Fused2Shape<PL, MODE_PFB, N1>::SMEM); if (rc) return rc; }
         // resident CTAs per SM: 128 registers x 512 threads fill the register file, 4 x 64 (2 x 128) TMEM
         // columns and 4 x 33 KB of shared memory fit.  The occupancy API cannot be asked: it reports 1
         // for any kernel that contains tcgen05.alloc (measured: 4 such CTAs of 128 threads do share an
@@ -856,9 +861,10 @@ static int fused_do(spec_ctx* s, bool query, const InputView& view, long long ns
             ProfScope ps(s, 0, st);
             if (tc) CK(cudaLaunchKernelEx(&cfg, kern_tc, p));
             else if constexpr (kF2) {
-                cfg.gridDim = dim3(2 * s->numSM); cfg.blockDim = dim3(256);
-                cfg.dynamicSmemBytes = Fused2Shape<PL, MODE_PFB>::SMEM;
-                CK(cudaLaunchKernelEx(&cfg, k_fused2<PL, MODE_PFB>, p));
+                typedef Fused2Shape<PL, MODE_PFB, N1> SH2;
+                cfg.gridDim = dim3((256 / SH2::NT) * s->numSM); cfg.blockDim = dim3(2 * SH2::NT);
+                cfg.dynamicSmemBytes = SH2::SMEM;
+                CK(cudaLaunchKernelEx(&cfg, k_fused2<PL, MODE_PFB, N1>, p));
             } else CK(cudaLaunchKernelEx(&cfg, kern, p));
         }
         CK(cudaGetLastError());
@@ -902,8 +908,21 @@ static int fused_dispatch(spec_ctx* s, bool query, const InputView& view, long l
 
 // `nspec` spectra starting at view-spectrum m0; c0 = spectra produced before them (window bookkeeping
 // is done inside the kernels, so a launch may span accumulation windows)
+// Packet-sized calls: a persistent launch costs about 8-11 us however little it has to do
+// (every CTA of a whole-GPU grid allocates tensor memory, waits for all the others, carries history, drains); below this many
+// samples the same 16 x N2 plan runs as two ordinary launches instead (pass A into the Z ring's memory, pass B out of it):
+// same intermediate layout, same accumulator order, so calls of both kinds mix freely on one handle.
+static bool small_call(const spec_ctx* s, long long nspec) {
+    return s->fused && s->N1 == 16 && !s->dump && !s->tc_stage && nspec * (long long)s->N <= (1ll << 18) && nspec <= s->zbatch;
+}
+
 static int run_spectra(spec_ctx* s, const InputView& v, long long m0, long long nspec, long long c0, cudaStream_t st) {
     if (s->N1 == 1) return run_single(s, v, m0, nspec, c0, st);
+    if (small_call(s, nspec) && (s->mode == SPEC_MODE_PFB || !s->use_coef)) {
+        int rc = run_passA(s, v, m0, (int)nspec, st);
+        if (rc) return rc;
+        return run_passB(s, (int)nspec, c0, st);
+    }
     if (s->r2_single) return s->use_coef ? launch_single_r2<PL4096, 1>(s, v, nspec, c0, st) : launch_single_r2<PL4096, 0>(s, v, nspec, c0, st);
     if (s->fused && (s->mode == SPEC_MODE_PFB || !s->use_coef)) return fused_dispatch(s, false, v, nspec, c0, st);
     for (long long b0 = 0; b0 < nspec; b0 += s->zbatch) {
@@ -1392,7 +1411,7 @@ extern "C" int spec_process(spec_t* s, const void* d_in, size_t nsamples, void* 
     const long long keep = total < T - 1 ? total : T - 1;
     bool carried = false;
     if (nspec > 0) {
-        if (s->fused && s->N1 > 1 && keep > 0 && nblk >= keep && (s->mode == SPEC_MODE_PFB || !s->use_coef)) {
+        if (s->fused && s->N1 > 1 && keep > 0 && nblk >= keep && (s->mode == SPEC_MODE_PFB || !s->use_coef) && !small_call(s, nspec)) {
             const size_t bb = block_bytes(s);
             s->carry_src = (const uint8_t*)d_in + (size_t)(nblk - keep) * bb;
             s->carry_dst = s->d_hist[nxt];
@@ -1670,10 +1689,15 @@ extern "C" int spec_plan_info(const spec_t* s, int* n1, int* n2, char* desc, siz
             snprintf(desc, desc_len, "k_engine<Plan<%d,%d,%d,%d>> single CTA per spectrum: unpack%s+FFT+Stokes+accumulate",
                      s->N2, r[0], r[1], r[2], pfb ? "+FIR" : (s->use_coef ? "+window" : ""));
         else if (s->fused && (pfb || !s->use_coef))
-            snprintf(desc, desc_len, "k_fused<Plan<%d,%d,%d,%d>,%d,%s> persistent four-step %dx%d: unpack%s+FFT+Stokes+accumulate, "
-                     "grid %d, Z ring %d groups x %d spectra",
-                     s->N2, r[0], r[1], r[2], s->N2 == 4096 ? 256 : 128, pfb ? "PFB" : "FFT", s->N1, s->N2,
-                     pfb ? "+FIR" : "", s->fgrid, s->fRING, s->fGS);
+        {
+            // (mirrors fused_do's kF2: three-stage row plans; FFT mode, or PFB with 4096-point rows, if the buffers fit)
+            const bool f2 = s->N2 >= 512 && (!pfb || s->N2 == 4096) && !(pfb && s->N1 == 128) && !s->tc_stage;
+            snprintf(desc, desc_len, "%s<Plan<%d,%d,%d,%d>,%s> persistent four-step %dx%d: unpack%s+FFT+Stokes+accumulate, "
+                     "%s, Z ring %d groups x %d spectra",
+                     f2 ? "k_fused2" : "k_fused", s->N2, r[0], r[1], r[2], pfb ? "PFB" : "FFT", s->N1, s->N2, pfb ? "+FIR" : "",
+                     f2 ? "one producer and one consumer group per CTA, rows prefetched by bulk copy" : "producer and consumer CTAs",
+                     s->fRING, s->fGS);
+        }
         else
             snprintf(desc, desc_len, "two-launch four-step %dx%d: %s then k_engine<Plan<%d,%d,%d,%d>> pass B, Z batch %d spectra",
                      s->N1, s->N2,

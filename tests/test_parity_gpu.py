@@ -336,7 +336,9 @@ def test_back_to_back_calls_without_sync(nchan, mode):
     torch, sp = _torch(), _sp()
     T = 8 if mode == PFB else 1
     M = 11
-    sizes = [9, 7, 12, 8, 10, 7]
+    mult = (1 << 18) // (7 * nchan) + 1      # every call above the small-call threshold: six persistent launches
+    sizes = [9 * mult, 7 * mult, 12 * mult, 8 * mult, 10 * mult, 7 * mult]
+    M = 11 * mult
     nblk = sum(sizes)
     raw = synth.dual_pol_stream(700 + nchan // 1024 + mode, nblk * nchan, [synth.F_CFG1])
     r, rd = oracle_run(raw, nchan, T, 2, mode, M, window=(1 if mode == PFB else 0))
@@ -366,12 +368,13 @@ def test_soak_random_call_sizes_two_handles_and_a_foreign_kernel():
     blocks of history, so both history-carry paths alternate), two handles on two streams, and a foreign kernel
     that takes every SM's shared memory for 50 ms in the middle of it on a third stream."""
     torch, sp = _torch(), _sp()
-    cfgs = [(8192, PFB, 8, 97), (32768, FFT, 1, 64), (1024, PFB, 8, 500)]
+    cfgs = [(8192, PFB, 8, 397), (32768, FFT, 1, 64), (1024, PFB, 8, 5000)]
     rng = np.random.default_rng(2026)
     ncalls = 220
     plans, raws, specs, devs = [], [], [], []
     for i, (N, mode, T, M) in enumerate(cfgs):
-        sizes = rng.integers(1, 25, size=ncalls)
+        big = (1 << 19) // N + 25               # calls on both sides of the small-call threshold (2^18 samples)
+        sizes = rng.integers(1, big, size=ncalls)
         sizes[rng.integers(0, ncalls, size=40)] = rng.integers(1, 7, size=40)   # plenty of calls below T-1 blocks
         plans.append(sizes)
         raws.append(synth.dual_pol_stream(1200 + i, int(sizes.sum()) * N, [synth.F_CFG1]))
