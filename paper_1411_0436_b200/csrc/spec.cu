@@ -777,11 +777,11 @@ template <class PL, int NT, int MODE_PFB, int PER_SM, int N1 = 16>
 static int fused_do(spec_ctx* s, bool query, const InputView& view, long long nspec, long long c0, cudaStream_t st) {
     constexpr bool kTcOk = (MODE_PFB == 0 && N1 == 16 && NT == 128);   // plans that have a tensor-core first stage
     // plans that run as k_fused2 (both roles per CTA, consumer rows prefetched by bulk copy): direct-FFT mode, and PFB mode
-    // where rows are 4096 points (N >= 65536: the ring misses the L2 there and the prefetch hides DRAM latency) and the
-    // producer's buffers leave room for two row buffers.  Measured (profiles/r02_experiments.md): FFT 16384 / 32768
+    // at N = 131072 and 262144 (the ring misses the L2 there and the prefetch hides DRAM latency; at 524288 the producer's
+    // buffers leave no room for two row buffers, at 65536 it measured slower: sweep 104.8 -> 88.6 GHz).  Measured (profiles/r02_experiments.md): FFT 16384 / 32768
     // 136 -> 149 / 146 GHz, PFB 131072 / 262144 71 -> 82 / 58 -> 71 GHz, but PFB 32768 117 -> 108 GHz (the staged rows add a
     // shared-memory pass to a mode whose shared-memory pipe is already half busy with the FIR hand-off)
-    constexpr bool kF2 = PL::NST == 3 && Fused2Shape<PL, MODE_PFB, N1>::kFits && (MODE_PFB == 0 || NT == 256);
+    constexpr bool kF2 = PL::NST == 3 && Fused2Shape<PL, MODE_PFB, N1>::kFits && (MODE_PFB == 0 || (NT == 256 && N1 > 16));
     auto kern = k_fused<PL, NT, MODE_PFB, PER_SM, false, N1>;
     auto kern_tc = k_fused<PL, NT, MODE_PFB, PER_SM, false, N1, kTcOk>;
     // exchange buffer / FIR hand-off, plus (PFB) the staged raw tile of a producer phase: R+7 blocks of 1 KiB
@@ -1691,7 +1691,7 @@ extern "C" int spec_plan_info(const spec_t* s, int* n1, int* n2, char* desc, siz
         else if (s->fused && (pfb || !s->use_coef))
         {
             // (mirrors fused_do's kF2: three-stage row plans; FFT mode, or PFB with 4096-point rows, if the buffers fit)
-            const bool f2 = s->N2 >= 512 && (!pfb || s->N2 == 4096) && !(pfb && s->N1 == 128) && !s->tc_stage;
+            const bool f2 = s->N2 >= 512 && (!pfb || (s->N2 == 4096 && s->N1 > 16)) && !(pfb && s->N1 == 128) && !s->tc_stage;
             snprintf(desc, desc_len, "%s<Plan<%d,%d,%d,%d>,%s> persistent four-step %dx%d: unpack%s+FFT+Stokes+accumulate, "
                      "%s, Z ring %d groups x %d spectra",
                      f2 ? "k_fused2" : "k_fused", s->N2, r[0], r[1], r[2], pfb ? "PFB" : "FFT", s->N1, s->N2, pfb ? "+FIR" : "",

@@ -726,6 +726,27 @@ def test_config3_pfb_512k_four_step():
 def test_config1_pfb_32k_streamed_64MiB_calls():
     g, r, _ = _run_config(1)
     assert len(g) == 7  # 2041 spectra, M=256: windows straddle the 64 MiB calls
+    # the call pattern bench.py times: the four 64 MiB calls queued back to back (overlapping persistent launches,
+    # history handed over inside the kernels), no read and no synchronisation in between, ONE batched read-out at the end
+    torch, sp = _torch(), _sp()
+    c = synth.CONFIGS[1]
+    raw = synth.config_stream(1)
+    d = torch.from_numpy(raw.reshape(-1)).cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    s = sp.Spec(c["nchan"], c["ntaps"], 2, PFB, c["nacc"], 1)
+    s.set_ring(16)
+    out = torch.zeros((16, 4, c["nchan"]), dtype=torch.float32, device="cuda")
+    per = c["nsamples"] // c["calls"]
+    for rep in range(3):
+        torch.cuda.synchronize()
+        for k in range(c["calls"]):
+            s.process(d.data_ptr() + k * per * 4, per, st)
+        assert s.read_accum_batch_device(out.data_ptr(), 16, st) == 7
+        got = out[:7].cpu().numpy()
+        for a, b in zip(got, r):
+            compare(a, b, f"configs[1], bench.py's call pattern, repetition {rep}")
+        s.reset()
+    s.close()
 
 
 # ---------------------------------------------------------------- API behaviour on the device
