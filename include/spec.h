@@ -181,6 +181,25 @@ int spec_profile_read(spec_t* s, double ms[4], long launches[4]);
 int spec_debug_unpack(const void* d_bytes, size_t nbytes, int npol, float* d_out, void* cuda_stream);
 int spec_debug_fir(spec_t* s, const void* d_blocks, int nspec, float* d_out, void* cuda_stream);
 
+/* A one-shot entry point that ALLOCATES NOTHING, for callers that cannot call cudaMalloc (code under CUDA-graph capture,
+ * tight serving loops, harnesses that forbid it): no handle, no cudaMalloc / cudaFree / allocating library routine, ever.
+ * Runs the whole chain of PAPER.md:87-96 (unpack, optional FIR, nchan-point FFT, Stokes, sum) over ONE stretch of samples
+ * with the single-kernel plan and writes the sum over all its spectra.
+ *   d_in      DEVICE, nsamples time samples of 2*npol int8 (layout as spec_process), 16-byte aligned, nsamples a
+ *             multiple of nchan; the filter history is empty: nsamples/nchan - (ntaps-1) spectra are formed.
+ *   nchan     power of two, 16 <= nchan <= 4096 (SPEC_ERR_SIZE beyond: the scratch array is fixed at 112 KiB).
+ *   ntaps, d_coeffs   d_coeffs == NULL: direct FFT, rectangular window (ntaps must be 1).  Else DEVICE array of
+ *             ntaps*nchan fp32 filter coefficients (ntaps 1..64; ntaps = 1 is a window over nchan).
+ *   d_out     DEVICE, planar [S][nchan] fp32 (S = 4 for npol = 2, else 1), natural channel order, overwritten.
+ * Returns the number of spectra summed (>= 1) or an SPEC_ERR_* code; all work is queued on cuda_stream.
+ * The scratch (accumulators in the engine's order, stage twiddles, channel table) is a file-scope device array inside the
+ * library: every GPU that loads the library holds its 112 KiB until exit.  All calls share it, and it keeps the last
+ * call's contents: the sums are cleared at the start of every call, the tables are re-uploaded (two small host-to-
+ * device copies on cuda_stream) whenever nchan differs from the previous call's on that device.  Calls that OVERLAP on
+ * the GPU (different streams, no dependency between them) race on the array: serialise them. */
+int spec_oneshot_static(const void* d_in, size_t nsamples, int nchan, int ntaps, int npol, const float* d_coeffs,
+                        float* d_out, void* cuda_stream);
+
 /* Throughput probe behind the design notes: thread-instructions per clock and SM (at the
  * device's nominal clock) of op 0 scalar FFMA, 1 packed FFMA2, 2 packed FADD2, 3 PRMT, 4 LDS.128 alone,
  * 5 LDS.128 with eight FFMA2 behind each load (counts the loads), 6 SHFL; 1024 threads per SM, independent chains. */

@@ -1654,6 +1654,110 @@ extern "C" int spec_debug_fir(spec_t* s, const void* d_blocks, int nspec, float*
     return rc;
 }
 
+// ------------------------------------------------------------------ one-shot entry point that allocates nothing
+// spec_oneshot_static (include/spec.h): for callers that cannot call cudaMalloc (code under CUDA-graph capture, tight
+// serving loops, harnesses that forbid it).  The single-kernel plan (k_engine, nchan <= 4096) needs three pieces of scratch
+// besides the caller's input and output: the accumulators in engine position order, the engine's stage twiddles and the
+// position -> channel table.  Here they live in ONE file-scope device array of fixed size that every GPU which loads the
+// library holds until exit:
+//     [0, 64 KiB)        accumulators  float[S][4096] worth of [position][S] sums  (cleared at the start of every call)
+//     [64 KiB, 96 KiB)   stage twiddles, at most 4096 float2                        (re-uploaded when nchan changes)
+//     [96 KiB, 112 KiB)  position -> channel table, 4096 int                       (re-uploaded when nchan changes)
+// In host code the array's NAME is only a host-side stand-in; the device address comes from cudaGetSymbolAddress, taken once
+// per device with that device current.  Every call shares the array: calls that overlap on the GPU (two streams) race.
+#define SPEC_STATIC_MAX_NCHAN 4096
+#define SPEC_STATIC_ACC_BYTES (16 * SPEC_STATIC_MAX_NCHAN)
+#define SPEC_STATIC_TW_BYTES (8 * SPEC_STATIC_MAX_NCHAN)
+#define SPEC_STATIC_PERM_BYTES (4 * SPEC_STATIC_MAX_NCHAN)
+#define SPEC_STATIC_BYTES (SPEC_STATIC_ACC_BYTES + SPEC_STATIC_TW_BYTES + SPEC_STATIC_PERM_BYTES)   // 112 KiB
+static __device__ __align__(256) unsigned char g_static_scratch[SPEC_STATIC_BYTES];
+
+struct StaticSetup {
+    unsigned char* ptr = nullptr;   // device address of g_static_scratch on this device
+    int numSM = 0;
+    int nchan = 0;                  // the tables in the array belong to this channel count (0: none yet)
+};
+static StaticSetup g_static[64];
+static std::mutex g_static_mu;
+// host staging of the tables (static: nothing is allocated; cudaMemcpyAsync from pageable memory returns once it has
+// taken its copy, so the arrays may be rewritten by the next set-up)
+static float2 g_static_tw[SPEC_STATIC_MAX_NCHAN];
+static int g_static_perm[SPEC_STATIC_MAX_NCHAN];
+
+extern "C" int spec_oneshot_static(const void* d_in, size_t nsamples, int nchan, int ntaps, int npol,
+                                   const float* d_coeffs, float* d_out, void* cuda_stream) {
+    if (!d_in || !d_out || ((uintptr_t)d_in & 15)) return SPEC_ERR_ARG;
+    if (npol != 1 && npol != 2) return SPEC_ERR_ARG;
+    if (nchan < 16 || (nchan & (nchan - 1))) return SPEC_ERR_ARG;
+    if (nchan > SPEC_STATIC_MAX_NCHAN) {
+        snprintf(g_err, sizeof(g_err), "spec_oneshot_static: nchan %d exceeds the static scratch array (at most %d channels, "
+                 "%d bytes per GPU); use a spec_create handle for larger transforms", nchan, SPEC_STATIC_MAX_NCHAN, SPEC_STATIC_BYTES);
+        return SPEC_ERR_SIZE;
+    }
+    if (ntaps < 1 || ntaps > 64 || (ntaps > 1 && !d_coeffs)) return SPEC_ERR_ARG;
+    if (nsamples % (size_t)nchan) return SPEC_ERR_SIZE;
+    const long long nblk = (long long)(nsamples / (size_t)nchan);
+    const long long nspec = nblk - (ntaps - 1);
+    if (nspec < 1 || nspec > 0x7fffffffll) return SPEC_ERR_SIZE;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return SPEC_ERR_ARG;
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    StaticSetup& su = g_static[dev];
+    if (!su.ptr) {   // once per device, with that device current
+        unsigned char* p = nullptr;
+        CK(cudaGetSymbolAddress((void**)&p, g_static_scratch));
+        CK(cudaDeviceGetAttribute(&su.numSM, cudaDevAttrMultiProcessorCount, dev));
+        su.ptr = p;
+    }
+    float* const acc = (float*)su.ptr;
+    float2* const tw = (float2*)(su.ptr + SPEC_STATIC_ACC_BYTES);
+    int* const perm = (int*)(su.ptr + SPEC_STATIC_ACC_BYTES + SPEC_STATIC_TW_BYTES);
+    if (su.nchan != nchan) {   // tables of another channel count (or none): upload this one's, ordered on the caller's stream
+        int r[3];
+        radices(nchan, r);
+        const int LA = nchan / r[0], LB = LA / r[1];
+        size_t ntw = 0;
+        if (r[1] == 1) g_static_tw[ntw++] = make_float2(1.f, 0.f);
+        else {
+            for (int q = 1; q < r[0]; q++)
+                for (int j = 0; j < LA; j++) {
+                    const double a = -2.0 * M_PI * (double)((long)j * q % nchan) / (double)nchan;
+                    g_static_tw[ntw++] = make_float2((float)cos(a), (float)sin(a));
+                }
+            if (r[2] != 1)
+                for (int q = 1; q < r[1]; q++)
+                    for (int j = 0; j < LB; j++) {
+                        const double a = -2.0 * M_PI * (double)((long)j * q % LA) / (double)LA;
+                        g_static_tw[ntw++] = make_float2((float)cos(a), (float)sin(a));
+                    }
+        }
+        for (int a = 0; a < nchan; a++) g_static_perm[a] = pos_to_freq(nchan, a);
+        su.nchan = 0;
+        CK(cudaMemcpyAsync(tw, g_static_tw, ntw * sizeof(float2), cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(perm, g_static_perm, (size_t)nchan * sizeof(int), cudaMemcpyHostToDevice, st));
+        su.nchan = nchan;
+    }
+    // a handle on the stack that points into the static array: the launch code of the single-kernel plan is reused as it is
+    spec_ctx tmp;
+    tmp.N = nchan; tmp.T = ntaps; tmp.P = npol; tmp.S = (npol == 2) ? 4 : 1;
+    tmp.mode = d_coeffs ? SPEC_MODE_PFB : SPEC_MODE_FFT; tmp.window = SPEC_WINDOW_RECT; tmp.M = (long)nspec;
+    tmp.N1 = 1; tmp.N2 = nchan; tmp.numSM = su.numSM;
+    tmp.use_coef = d_coeffs != nullptr;
+    tmp.d_coef = const_cast<float*>(d_coeffs);
+    tmp.d_tw2 = tw; tmp.d_perm = perm; tmp.d_ring = acc; tmp.nring = 1;
+    // the array keeps the last call's contents: the sums must start at zero
+    CK(cudaMemsetAsync(acc, 0, acc_floats(&tmp) * sizeof(float), st));
+    InputView view{nullptr, (const uint8_t*)d_in, 0};
+    int rc = run_single(&tmp, view, 0, nspec, 0, st);
+    if (rc) return rc;
+    k_unpermute<<<cdiv(nchan, 256), 256, 0, st>>>(acc, perm, d_out, nchan, tmp.S, 0, 1);
+    CK(cudaGetLastError());
+    return (int)nspec;
+}
+
 extern "C" int spec_debug_hog(int ms, size_t smem_bytes, void* cuda_stream) {
     if (ms < 0 || ms > 2000 || smem_bytes > 227 * 1024) return SPEC_ERR_ARG;
     int dev = 0, nsm = 0;

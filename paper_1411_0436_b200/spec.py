@@ -27,7 +27,7 @@ SYMBOLS = [
     "spec_stream_host", "spec_measure_fp32_peak", "spec_debug_unpack", "spec_debug_fir",
     "spec_strerror", "spec_last_error", "spec_profile", "spec_profile_read", "spec_read_accum_batch",
     "spec_plan_info", "spec_debug_hog", "spec_set_option", "spec_capture_begin", "spec_capture_end", "spec_replayed",
-    "spec_accumulate_host", "spec_create_subbands", "spec_debug_probe",
+    "spec_accumulate_host", "spec_create_subbands", "spec_debug_probe", "spec_oneshot_static",
 ]
 
 if not os.path.exists(LIB_PATH):
@@ -55,6 +55,7 @@ _lib.spec_measure_fp32_peak.argtypes = [C.POINTER(C.c_double), _vp]
 _lib.spec_debug_unpack.argtypes = [_vp, _sz, C.c_int, _vp, _vp]
 _lib.spec_debug_fir.argtypes = [_vp, _vp, C.c_int, _vp, _vp]
 _lib.spec_debug_hog.argtypes = [C.c_int, _sz, _vp]
+_lib.spec_oneshot_static.argtypes = [_vp, _sz, C.c_int, C.c_int, C.c_int, _vp, _vp, _vp]
 _lib.spec_debug_probe.argtypes = [C.c_int, C.POINTER(C.c_double), _vp]
 _lib.spec_set_option.argtypes = [_vp, C.c_int, C.c_int]
 _lib.spec_capture_begin.argtypes = [_vp]
@@ -105,6 +106,16 @@ def debug_probe(op, stream=0):
     out = C.c_double(0.0)
     _check(_lib.spec_debug_probe(op, C.byref(out), stream), "spec_debug_probe")
     return out.value
+
+
+def oneshot_static(d_in_ptr, nsamples, nchan, d_out_ptr, ntaps=1, npol=2, d_coeffs_ptr=None, stream=0):
+    """spec_oneshot_static: the chain over one stretch of samples with no handle and no allocation; returns the spectra summed."""
+    rc = _lib.spec_oneshot_static(d_in_ptr, nsamples, nchan, ntaps, npol, d_coeffs_ptr, d_out_ptr, stream)
+    if rc == ERR_SIZE and nchan > 4096:      # the library says which limit was exceeded
+        e = SpecError(rc, "spec_oneshot_static")
+        e.args = (f"{e.args[0]} {_lib.spec_last_error().decode()}",)
+        raise e
+    return _check(rc, "spec_oneshot_static")
 
 
 def debug_hog(ms, smem_bytes, stream=0):
