@@ -260,6 +260,7 @@ def run_ours(a):
     N, T, M, pfb = w["nchan"], w["ntaps"], w["nacc"], w["pfb"]
     cs = w["chunk_samples"]
     pass_samples = cs * CALLS_PER_PASS
+    READOUT_EVERY = a.readout_every
 
     # synthetic stream of configs[1] (config-1 generator), one pass long, per-rank seed
     raw = synth.dual_pol_stream(synth.SEED_BASE + 1 + 1000 * rank, pass_samples, [synth.F_CFG1])
@@ -516,12 +517,13 @@ def run_sweep(a):
                     times.append(e0.elapsed_time(e1))
                     s.reset()
                 res[name] = (1 << L) / (float(np.median(times)) * 1e-3) / 1e9
+                res[name + "_ms"] = [round(t, 3) for t in times]
             _, _, desc = s.plan_info()
             s.close()
             F = chain_flops_per_sample(N, T, pfb)
             roof = min(hbm / 4.0, fp32_peak * 1e3 / F)
             row = {"sweep_point": True, "mode": mode, "nchan": N, "ntaps": T, "nacc": M, "samples": 1 << L,
-                   "resident_ghz": res["resident"], "streamed_ghz": res["streamed"],
+                   "resident_ghz": res["resident"], "streamed_ghz": res["streamed"], "resident_runs_ms": res["resident_ms"],
                    "streamed_h2d_gbs": res["streamed"] * 4, "roof_ghz": roof, "frac": res["resident"] / roof,
                    "fp32_peak_tflops": fp32_peak, "plan": desc}
             rows.append(row)
@@ -605,6 +607,7 @@ def main():
     p.add_argument("--mode", default="pfb", choices=["pfb", "fft"])
     p.add_argument("--nacc", type=int, default=0)
     p.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    p.add_argument("--readout-every", type=int, default=READOUT_EVERY, help="passes between read-outs of the resident arm")
     p.add_argument("--nsub", type=int, default=1, help="eight-sub-band modes (PAPER.md:73): interleaved sub-bands per time sample")
     p.add_argument("--packets", action="store_true",
                    help="NEXT-4: packet-sized calls (8 blocks each), issued one by one and replayed as one CUDA graph")

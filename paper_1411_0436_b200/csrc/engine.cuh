@@ -505,6 +505,10 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
     typename Sink::State st;
     sink.init(st, tmem_base, 128);
     sink.begin(st);
+    // Programmatic dependent launch (accumulating single-kernel launches only, spec.cu sets the attribute): the next
+    // spec_process call's launch may fill the SM slots this grid's last wave frees one by one.  The two grids share
+    // nothing but the accumulators (commutative reductions) and read-only tables; a no-op for ordinary launches.
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     uint32_t ttw = 0;
     if (Sink::kTmem) {
         const int warp = tid >> 5;
@@ -666,6 +670,9 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
     }
 
     if (Sink::kAccumulates && !DUMP && slot_ok && j0 < j1) flush_all(wcur);
+    // (a grid that overlapped its predecessor's tail must not COMPLETE before it: whatever follows in the stream, a
+    // read-out for one, relies on stream order)
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (Sink::kTmem) tmem_free_cta<TCOLS>(tmem_base);
 }
 

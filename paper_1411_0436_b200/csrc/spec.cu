@@ -48,6 +48,14 @@ extern "C" const char* spec_strerror(int code) {
     }
 }
 
+#ifdef SPEC_TUNING
+// Tuning builds only (-DSPEC_TUNING, never the default build): plan parameters overridden from the environment.
+static int tuning_int(const char* name, int dflt, int lo, int hi) {
+    if (const char* e = getenv(name)) { const long v = atol(e); if (v >= lo && v <= hi) return (int)v; }
+    return dflt;
+}
+#endif
+
 // ------------------------------------------------------------------ handle
 struct spec_ctx {
     int N, T, P, S, mode, window;
@@ -412,6 +420,23 @@ static int blocks_by_smem(size_t smem, int cap) {
     return b < 1 ? 1 : (b > cap ? cap : b);
 }
 
+// accumulating single-kernel launches: consecutive ones may overlap (programmatic stream serialisation, engine.cuh)
+template <class K, class... Args>
+static cudaError_t launch_pdl(K kern, dim3 grid, int nt, size_t smem, cudaStream_t st, const spec_ctx* s, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = dim3(nt); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    int pdl = s->capturing ? 0 : 1;
+#ifdef SPEC_TUNING
+    pdl = tuning_int("SPEC_SINGLE_PDL", pdl, 0, 1);
+#endif
+    cfg.numAttrs = pdl;
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+
 template <class PL, int MODE_PFB, int P, int WIN>
 static int launch_single_w(spec_ctx* s, const InputView& view, long long m0, long long nspec, long long c0,
                            cudaStream_t st) {
@@ -425,7 +450,15 @@ static int launch_single_w(spec_ctx* s, const InputView& view, long long m0, lon
     FrontRaw<MODE_PFB, P, WIN> front{view, s->d_coef, s->N, s->T, 1, m0};
     Sink sink{s->d_ring, acc_floats(s), s->nring, PL::L, 0};
     const int resident = blocks_by_smem(smem, MINB);
-    const long long target = (long long)s->numSM * resident * 2 * G;
+    // one wave: exactly the CTAs the GPU holds at once, each with the longest possible run (the per-CTA prologue --
+    // tensor-memory allocation, twiddles, pipeline fill -- is paid once per run), and the next call's launch fills the
+    // slots as they free (programmatic dependent launch).  Measured against two waves at 64 MiB calls
+    // (profiles/r02_experiments.md): FFT 1024 / 2048 / 4096: 232 -> 298, 291 -> 320, 256 -> 282 GHz
+    int waves = 1;
+#ifdef SPEC_TUNING
+    waves = tuning_int("SPEC_SINGLE_WAVES", 1, 1, 8);
+#endif
+    const long long target = (long long)s->numSM * resident * waves * G;
     const int len = cdiv(nspec, target);
     const int nruns = cdiv(nspec, len);
     JobMap jm{nspec, len, nruns, 1, nruns, c0, s->M};
@@ -442,7 +475,7 @@ static int launch_single_w(spec_ctx* s, const InputView& view, long long m0, lon
     if (rc) return rc;
     {
         ProfScope ps(s, 0, st);
-        kern<<<dim3(cdiv(nruns, G)), NT, smem, st>>>(front, sink, jm, s->d_tw2, nullptr);
+        CK(launch_pdl(kern, dim3(cdiv(nruns, G)), NT, smem, st, s, front, sink, jm, (const float2*)s->d_tw2, (float*)nullptr));
     }
     CK(cudaGetLastError());
     return 0;
@@ -526,7 +559,11 @@ static int launch_single_r2(spec_ctx* s, const InputView& view, long long nspec,
     FrontRawR2<WIN> front{view, s->d_twN, s->d_coef, s->N, PL::L, 0};
     Sink sink{s->d_ring, acc_floats(s), s->nring, PL::L, 1};
     const int resident = blocks_by_smem(smem, MINB);
-    const long long target = (long long)s->numSM * resident * 2 / 2;   // runs (each run is two slots)
+    int waves2 = 1;   // one wave of CTAs, as in launch_single_w (FFT 8192: 198 -> 214 GHz against two)
+#ifdef SPEC_TUNING
+    waves2 = tuning_int("SPEC_R2_WAVES", 1, 1, 8);
+#endif
+    const long long target = (long long)s->numSM * resident * waves2 / 2;   // runs (each run is two slots, i.e. two CTAs)
     const int len = cdiv(nspec, target < 1 ? 1 : target);
     const int nruns = cdiv(nspec, len);
     JobMap jm{nspec, len, 2 * nruns, 1, nruns, c0, s->M};
@@ -543,7 +580,7 @@ static int launch_single_r2(spec_ctx* s, const InputView& view, long long nspec,
     if (rc) return rc;
     {
         ProfScope ps(s, 0, st);
-        kern<<<dim3(2 * nruns), NT, smem, st>>>(front, sink, jm, s->d_tw2, nullptr);
+        CK(launch_pdl(kern, dim3(2 * nruns), NT, smem, st, s, front, sink, jm, (const float2*)s->d_tw2, (float*)nullptr));
     }
     CK(cudaGetLastError());
     return 0;
@@ -695,14 +732,6 @@ static int run_passB(spec_ctx* s, int nb, long long c0, cudaStream_t st) {
     }
     return SPEC_ERR_ARG;
 }
-
-#ifdef SPEC_TUNING
-// Tuning builds only (-DSPEC_TUNING, never the default build): plan parameters overridden from the environment.
-static int tuning_int(const char* name, int dflt, int lo, int hi) {
-    if (const char* e = getenv(name)) { const long v = atol(e); if (v >= lo && v <= hi) return (int)v; }
-    return dflt;
-}
-#endif
 
 // ---- fused persistent four-step kernel (fused.cuh): one launch per call
 static const int FUSED_ROLE_WORDS = kFusedRoleWords;
