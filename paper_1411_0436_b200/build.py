@@ -19,7 +19,13 @@ DEPS = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith(("
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
-    "-split-compile", "0",   # optimise and assemble the kernels in parallel (2.5 min -> 1.4 min on 8 cores)
+    # Optimise and assemble the kernels in parallel, with a FIXED split and a source path relative to csrc/ so that the
+    # build is byte-for-byte reproducible wherever it runs.  This matters beyond hygiene: the compiler produces one of
+    # two code generations of the SAME source depending on how the kernels are partitioned (and, with "-split-compile
+    # 0", on the machine's core count and the repository's path): measured on one B200 (profiles/r02_experiments.md,
+    # row 24) split 3 gives 117.1 / 146.2 / 129.7 / 70.7 GHz at PFB 32768, FFT 32768, PFB 4096, PFB 262144, splits
+    # 2, 4, 5, 6, 8 give 110 / 138.2 / 124.3 / 62.7 (and 282 instead of 266 GHz at direct FFT 4096)
+    "-split-compile", "3",
 ]
 
 
@@ -34,7 +40,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
         extra = os.environ.get("SPEC_NVCC_EXTRA", "").split()   # e.g. -DSPEC_FUSED_DEBUG_COUNTERS
-        cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
+        cmd = ([nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB]
+               + [os.path.relpath(p, CSRC) for p in SOURCES])
         subprocess.check_call(cmd, cwd=CSRC)
     return LIB
 
