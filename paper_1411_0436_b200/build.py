@@ -19,13 +19,11 @@ DEPS = [os.path.join(CSRC, f) for f in sorted(os.listdir(CSRC)) if f.endswith(("
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
     "-Xcompiler", "-fPIC", "-shared", "-cudart", "static",
-    # Optimise and assemble the kernels in parallel, with a FIXED split and a source path relative to csrc/ so that the
-    # build is byte-for-byte reproducible wherever it runs.  This matters beyond hygiene: the compiler produces one of
-    # two code generations of the SAME source depending on how the kernels are partitioned (and, with "-split-compile
-    # 0", on the machine's core count and the repository's path): measured on one B200 (profiles/r02_experiments.md,
-    # row 24) split 3 gives 117.1 / 146.2 / 129.7 / 70.7 GHz at PFB 32768, FFT 32768, PFB 4096, PFB 262144, splits
-    # 2, 4, 5, 6, 8 give 110 / 138.2 / 124.3 / 62.7 (and 282 instead of 266 GHz at direct FFT 4096)
-    "-split-compile", "3",
+    # NO "-split-compile": the parallel split is a race.  The same command line produced one of two code generations
+    # of the same source from run to run (measured on one B200, profiles/r02_experiments.md row 24: 117 or 110 GHz at
+    # configs[1], 146 or 138 GHz at direct FFT 32768, and the other way round 266 or 282 GHz at direct FFT 4096).
+    # Without it the build takes four minutes instead of one and a half, and is byte-for-byte reproducible; the source
+    # is named relative to csrc/ so that the repository's location does not enter the binary either.
 ]
 
 

@@ -442,6 +442,8 @@ struct JobMap {
                        // splits a spectrum over several slots, FrontRawR2)
     long long c0;      // spectrum count since stream start at job 0 (accumulation windows)
     long long M;       // spectra per accumulation window
+    int pdl = 0;       // 1: this launch lets the next launch of the stream start early (accumulating single-kernel plans only;
+                       // a pass-A / pass-B launch must NOT: what follows it reads or overwrites its Z)
 };
 
 
@@ -508,7 +510,7 @@ k_engine(const Front front, const Sink sink, const JobMap jm, const float2* __re
     // Programmatic dependent launch (accumulating single-kernel launches only, spec.cu sets the attribute): the next
     // spec_process call's launch may fill the SM slots this grid's last wave frees one by one.  The two grids share
     // nothing but the accumulators (commutative reductions) and read-only tables; a no-op for ordinary launches.
-    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    if (jm.pdl) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     uint32_t ttw = 0;
     if (Sink::kTmem) {
         const int warp = tid >> 5;

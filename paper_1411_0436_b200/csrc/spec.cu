@@ -461,7 +461,7 @@ static int launch_single_w(spec_ctx* s, const InputView& view, long long m0, lon
     const long long target = (long long)s->numSM * resident * waves * G;
     const int len = cdiv(nspec, target);
     const int nruns = cdiv(nspec, len);
-    JobMap jm{nspec, len, nruns, 1, nruns, c0, s->M};
+    JobMap jm{nspec, len, nruns, 1, nruns, c0, s->M, 1};
     if (s->dump) {   // test hook: the same kernel, front end only
         auto kd = k_engine<PL, false, G, MINB, FrontRaw<MODE_PFB, P, WIN>, Sink, true>;
         int rc = prep_smem(kd, smem);
@@ -566,7 +566,7 @@ static int launch_single_r2(spec_ctx* s, const InputView& view, long long nspec,
     const long long target = (long long)s->numSM * resident * waves2 / 2;   // runs (each run is two slots, i.e. two CTAs)
     const int len = cdiv(nspec, target < 1 ? 1 : target);
     const int nruns = cdiv(nspec, len);
-    JobMap jm{nspec, len, 2 * nruns, 1, nruns, c0, s->M};
+    JobMap jm{nspec, len, 2 * nruns, 1, nruns, c0, s->M, 1};
     if (s->dump) {
         auto kd = k_engine<PL, false, G, MINB, FrontRawR2<WIN>, Sink, true>;
         int rc = prep_smem(kd, smem);

@@ -93,3 +93,13 @@ def test_no_environment_switches_in_the_product_build():
             assert "abort(" not in code, f"{f}:{ln}: abort() in the library"
     from paper_1411_0436_b200 import build
     assert not any("SPEC_TUNING" in x for x in build.NVCC_FLAGS)
+
+
+def test_build_is_reproducible_by_construction():
+    """The library must come out byte-for-byte the same wherever it is built: no parallel split of the optimisation
+    (a race between two code generations, profiles/r02_experiments.md row 24) and no absolute path on the command line."""
+    from paper_1411_0436_b200 import build
+    assert "-split-compile" not in build.NVCC_FLAGS
+    assert "-lineinfo" in build.NVCC_FLAGS and "arch=compute_100a,code=sm_100a" in build.NVCC_FLAGS
+    src = open(build.__file__).read()
+    assert "os.path.relpath(p, CSRC)" in src
