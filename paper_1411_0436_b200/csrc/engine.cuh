@@ -318,6 +318,35 @@ __device__ __forceinline__ void tmem_free_cta(uint32_t base) {
         asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(base), "n"(NCOLS) : "memory");
 }
 
+// The persistent kernels (fused.cuh, fused2.cuh) allocate tensor memory ONLY in blocks of 128 columns, one per set of four
+// warps that needs one.  Their CTAs wait for one another, so a CTA blocked in tcgen05.alloc behind a CTA of its own grid
+// is a deadlock: with a single 256-column request per CTA, two foreign 128-column allocations (a pass-B launch of another
+// handle, say) on either side of the first CTA's block leave 256 free but not contiguous columns once they are gone, and
+// the second CTA of the SM never starts (seen once as a 10 s time-out in the soak test).  Requests of one size cannot
+// fragment: a free block of 128 always serves the next one.
+template <int NSETS>
+__device__ __forceinline__ void tmem_alloc_sets(uint32_t* slots_smem) {
+    if (threadIdx.x < 32) {
+#pragma unroll
+        for (int i = 0; i < NSETS; i++)
+            asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(slots_smem + i)), "n"(128) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+}
+template <int NSETS>
+__device__ __forceinline__ void tmem_free_sets(const uint32_t* slots_smem) {
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    __syncthreads();
+    if (threadIdx.x < 32) {
+#pragma unroll
+        for (int i = 0; i < NSETS; i++)
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*(volatile const uint32_t*)(slots_smem + i)), "n"(128) : "memory");
+    }
+}
+
 // dual-pol Stokes sink with the accumulators in tensor memory: column 4*q+{0,1,2,3} of the thread's
 // lane = XX, YY, Re, Im of its position 16*i+q
 struct SinkStokesTmem {
@@ -336,6 +365,11 @@ struct SinkStokesTmem {
     __device__ __forceinline__ void init(State& s, uint32_t tmem_base, int colstride = 64) const {
         const int warp = threadIdx.x >> 5;
         s.taddr = tmem_base + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * colstride);
+    }
+    // the thread's set of four warps owns the 128-column block at `set_base` (tmem_alloc_sets)
+    __device__ __forceinline__ void init_set(State& s, uint32_t set_base) const {
+        const int warp = threadIdx.x >> 5;
+        s.taddr = set_base + ((uint32_t)((warp & 3) * 32) << 16);
     }
     __device__ __forceinline__ void begin(State& s) const {
         float z[32];

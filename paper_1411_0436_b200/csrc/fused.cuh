@@ -621,11 +621,11 @@ k_fused(const FusedParams p) {
     constexpr int G = NT / NTS;                     // rows per B job
     constexpr int RGN = (G >= N1) ? 1 : N1 / G;     // row groups per spectrum (a spectrum has N1 rows)
     constexpr int SPJ = (G >= N1) ? G / N1 : 1;     // spectra per B job
-    constexpr int TCOLS = (NT > 128) ? 256 : 128;   // per set of four warps: 64 accumulator + 64 twiddle columns
+    constexpr int NSETS = NT / 128;                 // tensor memory: one block of 128 columns per set of four warps (64 accumulator + 64 twiddle columns)
     static_assert(NST >= 2 && PL::RLAST == 16 && G * L * 16 == NT * 256, "row plan");
     extern __shared__ float4 smem[];                // G*L float4: B exchange buffer / A FIR hand-off (+ the staged raw tile)
     __shared__ int s_role[2];
-    __shared__ uint32_t s_tmem;
+    __shared__ uint32_t s_tmem[NSETS];
 
     const int tid = threadIdx.x;
     const int GS = 1 << p.lgGS;
@@ -654,7 +654,9 @@ k_fused(const FusedParams p) {
     // Every CTA allocates its TMEM columns first, producers included: a CTA of a kernel that contains
     // tcgen05.alloc holds the SM's allocation permit until it relinquishes it, and (measured) no
     // further CTA of the grid is started on that SM before then.
-    const uint32_t tmem_base = tmem_alloc_cta<TCOLS>(&s_tmem);
+    tmem_alloc_sets<NSETS>(s_tmem);
+    const uint32_t tmem_base = *(volatile uint32_t*)&s_tmem[0];                    // (the tensor-core producer's tile: NT = 128)
+    const uint32_t tmem_mine = *(volatile uint32_t*)&s_tmem[threadIdx.x >> 7];     // my set's block
 
     // role and rank: the first na_per_sm CTAs to arrive on an SM produce, the others consume
     if (tid == 0) {
@@ -692,7 +694,6 @@ k_fused(const FusedParams p) {
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // No CTA may leave before every CTA of the grid has arrived: an early exit would free a slot on its
     // SM, a late CTA would land there as a fifth arrival and the per-SM role split would be off.
-    const uint32_t tmem_base_ = tmem_base;
     auto finish = [&]() {
         __syncthreads();
         // (the previous launch, if this one overlapped its tail, has completed long before any CTA gets here;
@@ -709,7 +710,7 @@ k_fused(const FusedParams p) {
             for (int i = tid; i < ngroups; i += NT) { p.a_done[i] = 0u; p.b_done[i] = 0u; }
             for (int i = tid; i < kFusedRoleWords; i += NT) p.role[i] = 0u;
         }
-        tmem_free_cta<TCOLS>(tmem_base_);
+        tmem_free_sets<NSETS>(s_tmem);
     };
     const bool is_a = s_role[0] != 0;
     const int rank = s_role[1];
@@ -804,7 +805,7 @@ k_fused(const FusedParams p) {
 
     SinkStokesTmem sink{p.ring, p.acc_stride, p.nring, L, 1};
     SinkStokesTmem::State st;
-    sink.init(st, tmem_base, 128);
+    sink.init_set(st, tmem_mine);
     sink.begin(st);
     // The stage twiddles a thread needs are the same for every job (they depend on its index only):
     // they are parked in tensor memory next to the accumulators (columns 64.. of the thread's lane) and

@@ -40,7 +40,7 @@ k_fused2(const FusedParams p) {
     typedef Fused2Shape<PL, MODE_PFB, N1> SH;
     constexpr int NT = SH::NT;
     constexpr int NTC = 2 * NT;                     // threads per CTA
-    constexpr int TCOLS = 2 * NT;                   // tensor-memory columns: the consumer warps use the upper half
+    constexpr int NSETS = NT / 128;                 // tensor memory: one block of 128 columns per set of four CONSUMER warps
     constexpr int L = PL::L, RA = PL::RA, RB = PL::RB, RC = PL::RC, NST = PL::NST;
     constexpr int LA = PL::LA, LB = PL::LB, NTS = PL::NTS;
     constexpr int G = SH::G;
@@ -48,7 +48,7 @@ k_fused2(const FusedParams p) {
     static_assert(NST == 3 && LB == 16 && RB == 16 && RC == 16 && LA % 128 == 0 && G >= 1 && G < N1, "three-stage row plan");
     extern __shared__ float4 smem[];
     float4* const rowbuf = (float4*)((uint8_t*)smem + SH::P_BYTES);   // [2][G*L]
-    __shared__ uint32_t s_tmem;
+    __shared__ uint32_t s_tmem[NSETS];
     __shared__ uint64_t s_full[2];
     __shared__ int s_last;
 
@@ -61,8 +61,9 @@ k_fused2(const FusedParams p) {
     const unsigned a_full = TPG;
     const unsigned rows_full = (unsigned)GS * (unsigned)N1;
 
-    // SinkStokesTmem addresses column block (warp >> 2) of 128 columns: the consumer warps use the upper half
-    const uint32_t tmem_base = tmem_alloc_cta<TCOLS>(&s_tmem);
+    // (blocks of 128 columns only: see tmem_alloc_sets in engine.cuh; the producer warps use none)
+    tmem_alloc_sets<NSETS>(s_tmem);
+    const uint32_t tmem_mine = *(volatile uint32_t*)&s_tmem[is_a ? 0 : (gtid - NT) >> 7];
     if (gtid == 0) {
         mbar_init(&s_full[0], 1);
         mbar_init(&s_full[1], 1);
@@ -136,7 +137,7 @@ k_fused2(const FusedParams p) {
 
         SinkStokesTmem sink{p.ring, p.acc_stride, p.nring, L, 1};
         SinkStokesTmem::State st;
-        sink.init(st, tmem_base, 128);
+        sink.init_set(st, tmem_mine);
         sink.begin(st);
         // the thread's stage twiddles, parked in tensor memory next to its accumulators (fused.cuh)
         constexpr int TWA = (16 / RA) * (RA - 1);
@@ -283,7 +284,11 @@ k_fused2(const FusedParams p) {
         for (int i = gtid; i < ngroups; i += NTC) { p.a_done[i] = 0u; p.b_done[i] = 0u; }
         for (int i = gtid; i < kFusedRoleWords; i += NTC) p.role[i] = 0u;
     }
-    if (gtid < 32) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base), "n"(TCOLS) : "memory");
+    if (gtid < 32) {
+#pragma unroll
+        for (int i = 0; i < NSETS; i++)
+            asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*(volatile uint32_t*)&s_tmem[i]), "n"(128) : "memory");
+    }
 }
 
 }  // namespace spk
